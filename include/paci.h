@@ -1,0 +1,240 @@
+/* paci.h -- C ABI of the B200-native PACI stage-step library (libpaci.so).
+ *
+ * PACI = Pipeline Asynchronous training with Controlled Inconsistency
+ * (/root/reference/PAPER.md; "P:n" below = line n of that file).
+ *
+ * The library implements the per-stage micro-batch step of Algorithm 1:
+ *   forward  F_i(h_{m,i-1}; theta_i)                       (Eq. 7; Alg. 1 lines 5-9)
+ *   backward g_{m,i}, grad h_{m,i-1} with the activations stashed at forward time and the
+ *            stage's CURRENT parameters                    (Eq. 1; Alg. 1 lines 11-15)
+ *   G_i += g_{m,i} in place, in fp32                        (Alg. 1 line 13)
+ *   one fused AdamW update every k local backwards          (Alg. 1 lines 16-19)
+ * under a per-stage parameter-version counter t and the admission rule q_i <= N-i
+ * (Eq. 9), and reports for every micro-batch the number of updates that fell between its
+ * forward and its backward, Delta_{m,i} = t^B - t^F (Eq. 8).
+ *
+ * Conventions
+ *   - plain C, no torch types.  Every pointer says HOST or DEVICE.  Sizes are in elements unless
+ *     they end in _bytes.  `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   - the library allocates NO device memory and creates NO streams for a stage: the caller owns
+ *     the workspace and every in/out buffer and must keep them alive until the enqueued work is done.
+ *   - all compute calls are asynchronous on `stream`; host counters advance at enqueue time, and the
+ *     per-stage stream order equals the call order, so host-side Delta equals device-side Delta.
+ *     A device-side stamp (a version word bumped by the AdamW kernel and sampled by the first kernel
+ *     of every forward/backward) is kept so that tests can prove it (paci_stage_device_stamps).
+ *   - return value: 0 (PACI_OK) or a negative error code; never throws.  paci_last_error() returns
+ *     a thread-local human-readable message for the last failing call.
+ *   - activations are row-major [mu, T, D] in the stage's compute dtype (float for PACI_FP32,
+ *     __nv_bfloat16 for PACI_BF16); tokens/targets are int32 [mu, T].
+ *   - stage_index s is 0-based; the paper's stage i is s+1, its N is n_stages, its a is k_accum.
+ */
+#ifndef PACI_H_
+#define PACI_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- error codes ------------------------------------------------------------------------ */
+#define PACI_OK       0
+#define PACI_EINVAL  (-1)  /* bad config / null or misaligned pointer / workspace too small          */
+#define PACI_EAGAIN  (-2)  /* admission rule refuses the forward: q_s > S-1-s (Alg. 1 line 5).       */
+                           /* State unchanged; retry after a backward.                               */
+#define PACI_ESTATE  (-3)  /* call out of protocol: backward for a micro-batch that is not the        */
+                           /* oldest unresolved forward (FIFO, R4); forward/backward while  */
+                           /* an update is pending (c == k and paci_maybe_step not yet called);       */
+                           /* mb_id reuse while unresolved.                                           */
+#define PACI_ECUDA   (-4)  /* CUDA error at launch; text in paci_last_error()                        */
+
+/* ---- dtypes ------------------------------------------------------------------------------ */
+#define PACI_FP32 0        /* fp32 activations, weights, FFMA GEMMs (parity mode, 1e-5)             */
+#define PACI_BF16 1        /* bf16 activations + bf16 weight shadow, tcgen05 GEMMs with fp32          */
+                           /* accumulation; fp32 master weights, m, v, G; fp32 LN/softmax statistics */
+
+/* ---- tensor groups for load/read ---------------------------------------------------------- */
+#define PACI_PARAM      0  /* fp32 master parameters theta_i                                        */
+#define PACI_GRAD_ACCUM 1  /* G_i: raw SUM of the window's gradients (the 1/k is applied in AdamW)    */
+#define PACI_ADAM_M     2
+#define PACI_ADAM_V     3
+
+typedef struct paci_stage paci_stage_t;       /* opaque host object */
+
+typedef struct paci_stage_config {
+  int32_t stage_index;   /* s, 0-based                                                            */
+  int32_t n_stages;      /* S (paper N).  Unresolved forwards allowed before admission: S-1-s     */
+  int32_t n_layers;      /* pre-LN GPT-2 decoder blocks on this stage (>= 0)                      */
+  int32_t d_model;       /* D, multiple of 8 (bf16: multiple of 64)                                */
+  int32_t n_heads;       /* H, D % H == 0; head dim 64 in PACI_BF16, any <= 128 in PACI_FP32      */
+  int32_t seq_len;       /* T                                                                      */
+  int32_t micro_batch;   /* mu sequences per micro-batch; M = mu*T tokens                          */
+  int32_t k_accum;       /* k (paper a): local backwards per optimizer update                      */
+  int32_t vocab;         /* V (used when has_embedding or has_head)                                */
+  int32_t has_embedding; /* stage holds wte, wpe and takes int32 tokens as input           */
+  int32_t has_head;      /* stage holds final LN + LM head + mean token cross-entropy.     */
+                         /* With has_embedding too the head is TIED to wte (one tensor, summed      */
+                         /* gradient); otherwise the stage owns its own copy "head.w" (DESIGN R10)  */
+  int32_t dtype;         /* PACI_FP32 | PACI_BF16                                                  */
+  float beta1, beta2, eps, weight_decay;   /* AdamW: 0.9, 0.95, 1e-8, 0.1 in the paper    */
+} paci_stage_config;
+
+/* Bytes of DEVICE workspace a stage with this config needs (parameters, m, v, G, bf16 shadow,
+ * S-s stash slots, scratch).  0 = invalid config (see paci_last_error). */
+size_t paci_stage_workspace_bytes(const paci_stage_config* cfg);
+
+/* Number of fp32 parameters of the stage (sum over tensors). 0 = invalid config. */
+size_t paci_stage_param_count(const paci_stage_config* cfg);
+
+/* Create a stage on the current CUDA device.  dev_ws: DEVICE, 256-byte aligned, >= workspace_bytes;
+ * borrowed until paci_stage_destroy.  Zeroes m, v, G and the counters on `stream`; parameters are
+ * undefined until paci_stage_load(PACI_PARAM, ...) has been called for every tensor. */
+int paci_stage_create(const paci_stage_config* cfg, void* dev_ws, size_t ws_bytes, void* stream,
+                      paci_stage_t** out);
+int paci_stage_destroy(paci_stage_t* st);
+
+/* Tensor names (stage-local): wte, wpe, h.<l>.ln1.g|b, h.<l>.attn.wqkv|bqkv|wo|bo, h.<l>.ln2.g|b,
+ * h.<l>.mlp.w1|b1|w2|b2, lnf.g|b, head.w (only when has_head && !has_embedding).
+ * Matrices are [out, in] row-major; wqkv rows are [q; k; v], head h = rows h*dh..(h+1)*dh-1 (R17).
+ * Returns the element count, or 0 if the stage has no such tensor. */
+size_t paci_stage_tensor_numel(const paci_stage_t* st, const char* name);
+
+/* Copy a HOST fp32 array of n elements into / out of one tensor of group `what`.
+ * load(PACI_PARAM) also refreshes the bf16 shadow.  Both synchronise `stream` before returning. */
+int paci_stage_load(paci_stage_t* st, int what, const char* name, const float* host_src, size_t n,
+                    void* stream);
+int paci_stage_read(paci_stage_t* st, int what, const char* name, float* host_dst, size_t n,
+                    void* stream);
+
+/* Forward of micro-batch mb_id (Alg. 1 lines 5-9).
+ *   in      DEVICE: int32 tokens [mu,T] if has_embedding, else h [mu,T,D] (compute dtype)
+ *   targets DEVICE: int32 [mu,T] if has_head, else NULL
+ *   out     DEVICE: h [mu,T,D] (compute dtype), or float loss[1] if has_head
+ * Admission: refused with PACI_EAGAIN when q_s > S-1-s.  On success records t^F = version, takes a
+ * stash slot, q_s += 1. */
+int paci_forward(paci_stage_t* st, int64_t mb_id, const void* in, const int32_t* targets, void* out,
+                 void* stream);
+
+/* Backward of micro-batch mb_id (Alg. 1 lines 11-15): must be the oldest unresolved forward.
+ *   dout DEVICE: grad wrt the stage output [mu,T,D] (compute dtype); NULL iff has_head
+ *   din  DEVICE: grad wrt the stage input  [mu,T,D]; NULL iff has_embedding
+ * Records Delta = version - t^F, accumulates weight gradients into G (fp32, in the GEMM epilogue),
+ * c_s += 1, q_s -= 1, frees the stash slot. */
+int paci_backward(paci_stage_t* st, int64_t mb_id, const void* dout, void* din, void* stream);
+
+/* Alg. 1 lines 16-19: if c_s == k enqueue ONE fused multi-tensor AdamW kernel (update theta with
+ * G/k and learning rate lr, refresh bf16 shadow, zero G, bump the device version word), then
+ * version += 1, c_s = 0.  Returns 1 if it stepped, 0 if not yet, < 0 on error.  This is the only
+ * call that changes parameters. */
+int paci_maybe_step(paci_stage_t* st, float lr, void* stream);
+
+int64_t paci_version(const paci_stage_t* st);          /* local updates applied so far (t)       */
+int32_t paci_unresolved(const paci_stage_t* st);       /* q_s                                          */
+int32_t paci_window_count(const paci_stage_t* st);     /* c_s                                          */
+/* Delta_{m,s} = t^B - t^F (Eq. 8) of a micro-batch whose backward has been enqueued;
+ * -1 if unknown (never forwarded, or backward not yet called).  The log keeps the last 4096 ids. */
+int32_t paci_crossed_updates(const paci_stage_t* st, int64_t mb_id);
+/* Device-side proof of the same numbers: versions sampled ON THE DEVICE by the first kernel of the
+ * forward and of the backward of mb_id.  Synchronises `stream`.  Returns 0 or PACI_EINVAL. */
+int paci_stage_device_stamps(paci_stage_t* st, int64_t mb_id, int64_t* vF, int64_t* vB, void* stream);
+
+const char* paci_last_error(void);
+
+/* ---- schedule driver: S emulated stages on ONE GPU (BASELINE.json item 6) ------------------ */
+#define PACI_MODE_PACI  0   /* asynchronous 1F1B + accumulation                         */
+#define PACI_MODE_FLUSH 1   /* synchronous 1F1B-flush comparator; stages must have   */
+                            /* been created with k_accum = m_f                                     */
+
+typedef struct paci_pipeline paci_pipeline_t;
+
+typedef struct paci_run_report {
+  float*   loss;        /* HOST [n_microbatches] or NULL: loss of every micro-batch                */
+  int32_t* delta;       /* HOST [S * n_microbatches] or NULL: Delta_{m,s} at [s*n + m]             */
+  int64_t* version;     /* HOST [S] or NULL: local update index per stage after the run            */
+  int32_t* max_q;       /* HOST [S] or NULL: largest unresolved-forward count seen per stage       */
+  int64_t  n_slots;     /* out: logical slots the canonical schedule took                          */
+  int64_t  n_launches;  /* out: kernels launched by the library during the run                     */
+  float    elapsed_ms;  /* out: device time, first op to last op (CUDA events)                     */
+} paci_run_report;
+
+/* Bytes of DEVICE workspace for the inter-stage queues (activation / gradient rings, token staging). */
+size_t paci_pipeline_workspace_bytes(paci_stage_t* const* stages, int32_t n_stages);
+/* Creates one non-blocking stream per stage plus the ring events.  stages[s] must have stage_index s. */
+int paci_pipeline_create(paci_stage_t* const* stages, int32_t n_stages, void* dev_ws, size_t ws_bytes,
+                         paci_pipeline_t** out);
+int paci_pipeline_destroy(paci_pipeline_t* p);
+/* Run n_microbatches through the pipeline in the canonical logical schedule: per logical
+ * slot every stage does at most one op, a message produced in slot tau is visible in slot tau+1,
+ * backward before forward; the admission rule is enforced by paci_forward itself.
+ *   tokens: int32 [n_microbatches, mu, T+1]; column t+1 is the target of column t.
+ *           tokens_on_host = 0: DEVICE pointer.  1: HOST pointer (pinned or pageable); the run then
+ *           includes the host->device copy of every micro-batch's tokens and the device->host read
+ *           of its loss.
+ *   mode PACI_MODE_FLUSH: micro-batches are grouped k at a time and no forward of group g+1 is
+ *           issued at a stage before that stage applied update g.
+ * Blocks until the run is complete. */
+int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_on_host,
+                      int64_t n_microbatches, int32_t mode, float lr, paci_run_report* rep);
+
+/* ---- op-level entry points (kernel parity tests and per-kernel roofline measurements) ------ */
+/* All pointers DEVICE.  dtype = PACI_FP32 | PACI_BF16 selects the activation type T below. */
+
+/* GEMM  C[M,N] (+)= op(A) op(B) (+ bias).  lda, ldb, ldc = row strides in elements.  layout:
+ *   0 "NT" forward  : A[M,K] row-major, B[N,K] row-major (y = x W^T)         (SURVEY a3,a5,a7,a9,a10)
+ *   1 "NN" dgrad    : A[M,K] row-major, B[K,N] row-major (dx = dy W)         (a13, current W: Eq. 1)
+ *   2 "TN" wgrad    : A[K,M] row-major, B[K,N] row-major (dW = dy^T x)       (a14)
+ * out_f32_accum = 0: C is T, overwritten, bias (fp32 [N], may be NULL) added.
+ * out_f32_accum = 1: C is fp32 and the product is ADDED into it (beta = 1, Alg. 1 line 13).
+ * PACI_BF16: all leading dimensions and pointers must be multiples of 8 elements / 16 bytes. */
+int paci_op_gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
+                 const float* bias, void* C, int ldc, int out_f32_accum, void* stream);
+/* y = LN(x (+ res)) with gain g, bias b (fp32 [D]); writes xsum = x + res if xsum != NULL, and
+ * mean, rstd (fp32 [rows]).  (a2, a6) */
+int paci_op_layernorm_fwd(int dtype, int rows, int D, const void* x, const void* res, const float* g,
+                          const float* b, void* xsum, void* y, float* mean, float* rstd, void* stream);
+/* dx = (dres ? dres : 0) + LNbwd(dy; x, mean, rstd, g);  Gg += sum dy*xhat;  Gb += sum dy;
+ * if Gcol != NULL: Gcol += column sums of dx.  (a18, a15) */
+int paci_op_layernorm_bwd(int dtype, int rows, int D, const void* dy, const void* x, const float* mean,
+                          const float* rstd, const float* g, const void* dres, void* dx, float* Gg,
+                          float* Gb, float* Gcol, void* stream);
+int paci_op_gelu_fwd(int dtype, size_t n, const void* p, void* out, void* stream);          /* a8  */
+/* dp = dg * gelu'(p);  if Gbias != NULL: Gbias[cols] += column sums of dp.  (a16, a15) */
+int paci_op_gelu_bwd(int dtype, int rows, int cols, const void* dg, const void* p, void* dp,
+                     float* Gbias, void* stream);
+/* G[cols] += column sums of x[rows, cols].  (a15) */
+int paci_op_colsum(int dtype, int rows, int cols, const void* x, float* G, void* stream);
+/* Causal attention over packed qkv [mu,T,3D] -> o [mu,T,D], lse fp32 [mu,H,T].  (a4) */
+int paci_op_attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,
+                          void* stream);
+/* dqkv [mu,T,3D] from do, qkv, o, lse; scratch: fp32 [mu*H*T] (+ [mu*T*D] fp32 in bf16 mode). (a17) */
+int paci_op_attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
+                          const void* o, const float* lse, void* dqkv, float* scratch, void* stream);
+size_t paci_op_attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh);
+/* x = wte[tok] + wpe[pos] (a1);  tok int32 [mu,T]; wte, wpe fp32. */
+int paci_op_embed_fwd(int dtype, int mu, int T, int D, const int32_t* tok, const float* wte,
+                      const float* wpe, void* x, void* stream);
+/* Gwte[tok] += dx;  Gwpe[t] += sum_b dx  (a19). */
+int paci_op_embed_bwd(int dtype, int mu, int T, int D, const int32_t* tok, const void* dx, float* Gwte,
+                      float* Gwpe, void* stream);
+/* loss[0] += sum_rows (lse - z[tgt]) / rows;  z <- dz = (softmax(z) - onehot) / rows in place.
+ * z is [rows, ldz] with V valid columns (padding columns are written 0).  (a11) */
+int paci_op_softmax_ce(int dtype, int rows, int V, int ldz, void* z, const int32_t* tgt, float* loss,
+                       void* stream);
+/* Fused AdamW over a flat arena of n fp32 elements, the first n_decay of which decay (a20):
+ * g = G/k; w *= 1 - lr*wd (decayed part); m, v, bias-corrected update with step t; G = 0;
+ * shadow (bf16, may be NULL) = bf16(w); *version_word += 1 (may be NULL). */
+int paci_op_adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float* G, void* shadow_bf16,
+                  int k, int64_t t, float lr, float beta1, float beta2, float eps, float weight_decay,
+                  int64_t* version_word, void* stream);
+
+/* Number of kernels the library has launched in this process (for bench.py's gpu_launches). */
+int64_t paci_launch_count(void);
+/* 1 if the tcgen05 GEMM path is in use for PACI_BF16 GEMMs, 0 if the SIMT fallback was forced by
+ * the environment variable PACI_GEMM=simt (a debugging aid, never a silent fallback). */
+int paci_gemm_backend_is_tcgen05(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PACI_H_ */

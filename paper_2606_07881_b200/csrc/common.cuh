@@ -1,0 +1,146 @@
+// common.cuh -- shared device/host helpers of libpaci (sm_100a only).
+#pragma once
+
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <atomic>
+#include <cstdio>
+#include <string>
+
+#include "../../include/paci.h"
+
+namespace paci {
+
+// ---------------------------------------------------------------- error + launch bookkeeping
+extern thread_local std::string g_last_error;
+extern std::atomic<int64_t> g_launches;
+
+int fail(int code, const char* fmt, ...);
+
+#define PACI_CUDA_OK(expr)                                                              \
+  do {                                                                                  \
+    cudaError_t e__ = (expr);                                                           \
+    if (e__ != cudaSuccess)                                                             \
+      return ::paci::fail(PACI_ECUDA, "%s:%d %s -> %s", __FILE__, __LINE__, #expr,      \
+                          cudaGetErrorString(e__));                                     \
+  } while (0)
+
+// every kernel launch goes through this so that paci_launch_count() is exact
+#define PACI_LAUNCH(kernel, grid, block, smem, stream, ...)                             \
+  do {                                                                                  \
+    kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);                         \
+    ::paci::g_launches.fetch_add(1, std::memory_order_relaxed);                         \
+    PACI_CUDA_OK(cudaPeekAtLastError());                                                \
+  } while (0)
+
+// ---------------------------------------------------------------- dtype traits
+typedef __nv_bfloat16 bf16;
+
+template <typename T> struct Vec;                 // 16-byte vector of T
+template <> struct Vec<float> { static constexpr int N = 4; };
+template <> struct Vec<bf16>  { static constexpr int N = 8; };
+
+__device__ __forceinline__ float to_f(float x) { return x; }
+__device__ __forceinline__ float to_f(bf16 x) { return __bfloat162float(x); }
+template <typename T> __device__ __forceinline__ T from_f(float x);
+template <> __device__ __forceinline__ float from_f<float>(float x) { return x; }
+template <> __device__ __forceinline__ bf16 from_f<bf16>(float x) { return __float2bfloat16_rn(x); }
+
+// 16-byte global load / store of Vec<T>::N elements, converted to / from fp32 registers
+template <typename T> __device__ __forceinline__ void load_vec(const T* p, float (&v)[Vec<T>::N]);
+template <> __device__ __forceinline__ void load_vec<float>(const float* p, float (&v)[4]) {
+  float4 t = *reinterpret_cast<const float4*>(p);
+  v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+}
+template <> __device__ __forceinline__ void load_vec<bf16>(const bf16* p, float (&v)[8]) {
+  uint4 t = *reinterpret_cast<const uint4*>(p);
+  const __nv_bfloat162* h = reinterpret_cast<const __nv_bfloat162*>(&t);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    float2 f = __bfloat1622float2(h[i]);
+    v[2 * i] = f.x; v[2 * i + 1] = f.y;
+  }
+}
+template <typename T> __device__ __forceinline__ void store_vec(T* p, const float (&v)[Vec<T>::N]);
+template <> __device__ __forceinline__ void store_vec<float>(float* p, const float (&v)[4]) {
+  *reinterpret_cast<float4*>(p) = make_float4(v[0], v[1], v[2], v[3]);
+}
+template <> __device__ __forceinline__ void store_vec<bf16>(bf16* p, const float (&v)[8]) {
+  uint4 t;
+  __nv_bfloat162* h = reinterpret_cast<__nv_bfloat162*>(&t);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]);
+  *reinterpret_cast<uint4*>(p) = t;
+}
+// N consecutive fp32 values (N = 4 or 8) as float4 loads
+template <int N> __device__ __forceinline__ void load_f32(const float* p, float (&v)[N]) {
+#pragma unroll
+  for (int i = 0; i < N / 4; ++i) {
+    float4 t = reinterpret_cast<const float4*>(p)[i];
+    v[4 * i] = t.x; v[4 * i + 1] = t.y; v[4 * i + 2] = t.z; v[4 * i + 3] = t.w;
+  }
+}
+
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+
+static inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
+static inline size_t align_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
+
+int num_sms();
+int stage_cfg_field(const ::paci_stage* st, int field);   // i-th int32 of the stage's paci_stage_config
+
+// ---------------------------------------------------------------- kernel launchers (host)
+// dtype: PACI_FP32 | PACI_BF16.  All return PACI_OK or a negative code.
+int ln_fwd(int dtype, int rows, int D, const void* x, const void* res, const float* g, const float* b,
+           void* xsum, void* y, float* mean, float* rstd, cudaStream_t s);
+int ln_bwd(int dtype, int rows, int D, const void* dy, const void* x, const float* mean, const float* rstd,
+           const float* g, const void* dres, void* dx, float* Gg, float* Gb, float* Gcol, cudaStream_t s);
+int gelu_fwd(int dtype, size_t n, const void* p, void* out, cudaStream_t s);
+int gelu_bwd(int dtype, int rows, int cols, const void* dg, const void* p, void* dp, float* Gbias,
+             cudaStream_t s);
+int colsum(int dtype, int rows, int cols, const void* x, float* G, cudaStream_t s);
+int embed_fwd(int dtype, int mu, int T, int D, const int32_t* tok, const float* wte, const float* wpe,
+              void* x, cudaStream_t s);
+int embed_bwd(int dtype, int mu, int T, int D, const int32_t* tok, const void* dx, float* Gwte,
+              float* Gwpe, cudaStream_t s);
+int softmax_ce(int dtype, int rows, int V, int ldz, void* z, const int32_t* tgt, float* loss,
+               cudaStream_t s);
+int adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float* G, void* shadow, int k, int64_t t,
+          float lr, float beta1, float beta2, float eps, float wd, int64_t* version_word, cudaStream_t s);
+int cast_shadow(size_t n, const float* w, void* shadow, cudaStream_t s);          // bf16 shadow of fp32
+int stamp_version(const int64_t* version_word, int64_t* dst, cudaStream_t s);     // *dst = *version_word
+int split_tokens(int mu, int T, const int32_t* tok_tp1, int32_t* inp, int32_t* tgt, cudaStream_t s);
+
+// GEMM: see paci_op_gemm in paci.h for layouts; lda/ldb/ldc are row strides in elements.
+// gemm() dispatches on dtype / backend.
+int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
+         const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s);
+int gemm_simt(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
+              const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s);
+int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
+            void* C, int ldc, int out_f32_accum, cudaStream_t s);
+bool gemm_backend_tcgen05();
+int add_vec(int dtype, size_t n, const void* a, const void* b, void* out, cudaStream_t s);  // out = a (+ b)
+
+int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,
+                  cudaStream_t s);
+int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv, const void* o,
+                  const float* lse, void* dqkv, float* scratch, cudaStream_t s);
+size_t attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh);
+int attention_fwd_simt(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,
+                       cudaStream_t s);
+int attention_bwd_simt(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
+                       const void* o, const float* lse, void* dqkv, float* scratch, cudaStream_t s);
+
+}  // namespace paci

@@ -1,0 +1,641 @@
+// elementwise.cu -- the HBM-bound kernels of the PACI stage step (SURVEY.md 8(a) rows a1, a2, a6, a8,
+// a11, a15, a16, a18, a19, a20).  All use 16-byte vector accesses, fp32 statistics and warp-shuffle
+// reductions; grids are sized from the SM count.
+#include <cmath>
+#include <cstdarg>
+
+#include "common.cuh"
+
+namespace paci {
+
+thread_local std::string g_last_error;
+std::atomic<int64_t> g_launches{0};
+
+int fail(int code, const char* fmt, ...) {
+  char buf[1024];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  g_last_error = buf;
+  return code;
+}
+
+int num_sms() {
+  static int n = 0;
+  if (n == 0) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+    if (n <= 0) n = 148;
+  }
+  return n;
+}
+
+static constexpr float LN_EPS = 1e-5f;              // DESIGN.md R13
+static constexpr float GELU_C = 0.7978845608028654f;  // sqrt(2/pi), R12
+static constexpr float GELU_A = 0.044715f;
+
+// =========================================================================== LayerNorm forward
+// One warp per row; the row lives in registers (NV 16-byte vectors per lane).  Optionally adds a
+// residual first and writes the sum (the new residual stream) -- rows a2/a6: "LN (+ residual fused)".
+template <typename T, int NV>
+__global__ void __launch_bounds__(256) ln_fwd_kernel(int rows, int D, const T* __restrict__ x,
+                                                     const T* __restrict__ res, const float* __restrict__ g,
+                                                     const float* __restrict__ b, T* __restrict__ xsum,
+                                                     T* __restrict__ y, float* __restrict__ mean_out,
+                                                     float* __restrict__ rstd_out) {
+  constexpr int V = Vec<T>::N;
+  const int lane = threadIdx.x & 31;
+  const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (row >= rows) return;
+  const int nvec = D / V;
+  const size_t base = (size_t)row * D;
+  float v[NV][V];
+  float sum = 0.f;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = lane + 32 * i;
+    if (c < nvec) {
+      load_vec<T>(x + base + (size_t)c * V, v[i]);
+      if (res != nullptr) {
+        float r[V];
+        load_vec<T>(res + base + (size_t)c * V, r);
+#pragma unroll
+        for (int j = 0; j < V; ++j) v[i][j] += r[j];
+      }
+      if (xsum != nullptr) {
+        store_vec<T>(xsum + base + (size_t)c * V, v[i]);
+        if (sizeof(T) == 2) {  // statistics must see the ROUNDED stream that backward will re-read
+#pragma unroll
+          for (int j = 0; j < V; ++j) v[i][j] = to_f(from_f<T>(v[i][j]));
+        }
+      }
+#pragma unroll
+      for (int j = 0; j < V; ++j) sum += v[i][j];
+    }
+  }
+  const float mean = warp_sum(sum) / (float)D;
+  float sq = 0.f;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    if (lane + 32 * i < nvec) {
+#pragma unroll
+      for (int j = 0; j < V; ++j) {
+        const float d = v[i][j] - mean;
+        sq += d * d;
+      }
+    }
+  }
+  const float rstd = rsqrtf(warp_sum(sq) / (float)D + LN_EPS);
+  if (lane == 0) {
+    mean_out[row] = mean;
+    rstd_out[row] = rstd;
+  }
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = lane + 32 * i;
+    if (c < nvec) {
+      float gg[V], bb[V], o[V];
+      load_f32<V>(g + (size_t)c * V, gg);
+      load_f32<V>(b + (size_t)c * V, bb);
+#pragma unroll
+      for (int j = 0; j < V; ++j) o[j] = (v[i][j] - mean) * rstd * gg[j] + bb[j];
+      store_vec<T>(y + base + (size_t)c * V, o);
+    }
+  }
+}
+
+template <typename T>
+static int ln_fwd_t(int rows, int D, const void* x, const void* res, const float* g, const float* b,
+                    void* xsum, void* y, float* mean, float* rstd, cudaStream_t s) {
+  constexpr int V = Vec<T>::N;
+  if (D % V != 0) return fail(PACI_EINVAL, "layernorm: D=%d not a multiple of %d", D, V);
+  const int nv = ceil_div(D / V, 32);
+  const int wpb = 8;
+  dim3 grid(ceil_div(rows, wpb)), block(wpb * 32);
+#define LN_CASE(N)                                                                                      \
+  case N:                                                                                               \
+    PACI_LAUNCH((ln_fwd_kernel<T, N>), grid, block, 0, s, rows, D, (const T*)x, (const T*)res, g, b,    \
+                (T*)xsum, (T*)y, mean, rstd);                                                           \
+    break;
+  switch (nv) {
+    LN_CASE(1) LN_CASE(2) LN_CASE(3) LN_CASE(4) LN_CASE(5) LN_CASE(6) LN_CASE(7) LN_CASE(8)
+    default: return fail(PACI_EINVAL, "layernorm: D=%d too large", D);
+  }
+#undef LN_CASE
+  return PACI_OK;
+}
+
+int ln_fwd(int dtype, int rows, int D, const void* x, const void* res, const float* g, const float* b,
+           void* xsum, void* y, float* mean, float* rstd, cudaStream_t s) {
+  if (rows <= 0) return PACI_OK;
+  return dtype == PACI_BF16 ? ln_fwd_t<bf16>(rows, D, x, res, g, b, xsum, y, mean, rstd, s)
+                            : ln_fwd_t<float>(rows, D, x, res, g, b, xsum, y, mean, rstd, s);
+}
+
+// =========================================================================== LayerNorm backward
+// dx = dres + rstd * (g*dy - mean(g*dy) - xhat * mean(g*dy*xhat)) with the CURRENT gain g (Eq. 1) and
+// xhat recomputed from the stashed x, mean, rstd (no parameter involved).  Each lane owns fixed
+// columns, so the column reductions Gg += sum dy*xhat, Gb += sum dy and (optionally) Gcol += sum dx
+// are register partials, combined per block through shared-memory atomics, one global atomic per
+// column per block.
+template <typename T, int NV>
+__global__ void __launch_bounds__(256) ln_bwd_kernel(int rows, int D, const T* __restrict__ dy,
+                                                     const T* __restrict__ x, const float* __restrict__ mean,
+                                                     const float* __restrict__ rstd,
+                                                     const float* __restrict__ g, const T* __restrict__ dres,
+                                                     T* __restrict__ dx, float* __restrict__ Gg,
+                                                     float* __restrict__ Gb, float* __restrict__ Gcol) {
+  constexpr int V = Vec<T>::N;
+  extern __shared__ float sm[];  // [3][D]
+  const int lane = threadIdx.x & 31;
+  const int wpb = blockDim.x >> 5;
+  const int nvec = D / V;
+  for (int i = threadIdx.x; i < 3 * D; i += blockDim.x) sm[i] = 0.f;
+  __syncthreads();
+  float gg[NV][V], pg[NV][V], pb[NV][V], pc[NV][V];
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = lane + 32 * i;
+#pragma unroll
+    for (int j = 0; j < V; ++j) pg[i][j] = pb[i][j] = pc[i][j] = 0.f;
+    if (c < nvec) load_f32<V>(g + (size_t)c * V, gg[i]);
+  }
+  const float invD = 1.f / (float)D;
+  for (int row = blockIdx.x * wpb + (threadIdx.x >> 5); row < rows; row += gridDim.x * wpb) {
+    const size_t base = (size_t)row * D;
+    const float mu = mean[row], rs = rstd[row];
+    float dyv[NV][V], xh[NV][V];
+    float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      const int c = lane + 32 * i;
+      if (c < nvec) {
+        load_vec<T>(dy + base + (size_t)c * V, dyv[i]);
+        load_vec<T>(x + base + (size_t)c * V, xh[i]);
+#pragma unroll
+        for (int j = 0; j < V; ++j) {
+          xh[i][j] = (xh[i][j] - mu) * rs;
+          pg[i][j] += dyv[i][j] * xh[i][j];
+          pb[i][j] += dyv[i][j];
+          dyv[i][j] *= gg[i][j];
+          s1 += dyv[i][j];
+          s2 += dyv[i][j] * xh[i][j];
+        }
+      }
+    }
+    s1 = warp_sum(s1) * invD;
+    s2 = warp_sum(s2) * invD;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      const int c = lane + 32 * i;
+      if (c < nvec) {
+        float o[V];
+#pragma unroll
+        for (int j = 0; j < V; ++j) o[j] = rs * (dyv[i][j] - s1 - xh[i][j] * s2);
+        if (dres != nullptr) {
+          float r[V];
+          load_vec<T>(dres + base + (size_t)c * V, r);
+#pragma unroll
+          for (int j = 0; j < V; ++j) o[j] += r[j];
+        }
+        store_vec<T>(dx + base + (size_t)c * V, o);
+        if (Gcol != nullptr) {
+#pragma unroll
+          for (int j = 0; j < V; ++j) pc[i][j] += to_f(from_f<T>(o[j]));  // sum of what was stored
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = lane + 32 * i;
+    if (c < nvec) {
+#pragma unroll
+      for (int j = 0; j < V; ++j) {
+        atomicAdd(&sm[c * V + j], pg[i][j]);
+        atomicAdd(&sm[D + c * V + j], pb[i][j]);
+        if (Gcol != nullptr) atomicAdd(&sm[2 * D + c * V + j], pc[i][j]);
+      }
+    }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < D; i += blockDim.x) {
+    atomicAdd(&Gg[i], sm[i]);
+    atomicAdd(&Gb[i], sm[D + i]);
+    if (Gcol != nullptr) atomicAdd(&Gcol[i], sm[2 * D + i]);
+  }
+}
+
+template <typename T>
+static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float* mean, const float* rstd,
+                    const float* g, const void* dres, void* dx, float* Gg, float* Gb, float* Gcol,
+                    cudaStream_t s) {
+  constexpr int V = Vec<T>::N;
+  if (D % V != 0) return fail(PACI_EINVAL, "layernorm_bwd: D=%d not a multiple of %d", D, V);
+  const int nv = ceil_div(D / V, 32);
+  const int wpb = 8;
+  int blocks = num_sms() * 2;
+  if (blocks > ceil_div(rows, wpb)) blocks = ceil_div(rows, wpb);
+  dim3 grid(blocks), block(wpb * 32);
+  const size_t smem = 3 * (size_t)D * sizeof(float);
+#define LNB_CASE(N)                                                                                     \
+  case N:                                                                                               \
+    PACI_LAUNCH((ln_bwd_kernel<T, N>), grid, block, smem, s, rows, D, (const T*)dy, (const T*)x, mean,  \
+                rstd, g, (const T*)dres, (T*)dx, Gg, Gb, Gcol);                                         \
+    break;
+  switch (nv) {
+    LNB_CASE(1) LNB_CASE(2) LNB_CASE(3) LNB_CASE(4) LNB_CASE(5) LNB_CASE(6)
+    default: return fail(PACI_EINVAL, "layernorm_bwd: D=%d too large", D);
+  }
+#undef LNB_CASE
+  return PACI_OK;
+}
+
+int ln_bwd(int dtype, int rows, int D, const void* dy, const void* x, const float* mean, const float* rstd,
+           const float* g, const void* dres, void* dx, float* Gg, float* Gb, float* Gcol, cudaStream_t s) {
+  if (rows <= 0) return PACI_OK;
+  return dtype == PACI_BF16 ? ln_bwd_t<bf16>(rows, D, dy, x, mean, rstd, g, dres, dx, Gg, Gb, Gcol, s)
+                            : ln_bwd_t<float>(rows, D, dy, x, mean, rstd, g, dres, dx, Gg, Gb, Gcol, s);
+}
+
+// =========================================================================== GELU
+__device__ __forceinline__ float gelu_f(float p) {
+  const float u = GELU_C * (p + GELU_A * p * p * p);
+  return 0.5f * p * (1.f + tanhf(u));
+}
+__device__ __forceinline__ float dgelu_f(float p) {
+  const float u = GELU_C * (p + GELU_A * p * p * p);
+  const float th = tanhf(u);
+  return 0.5f * (1.f + th) + 0.5f * p * (1.f - th * th) * GELU_C * (1.f + 3.f * GELU_A * p * p);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) gelu_fwd_kernel(size_t nvec, const T* __restrict__ p, T* __restrict__ out) {
+  constexpr int V = Vec<T>::N;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    float v[V];
+    load_vec<T>(p + i * V, v);
+#pragma unroll
+    for (int j = 0; j < V; ++j) v[j] = gelu_f(v[j]);
+    store_vec<T>(out + i * V, v);
+  }
+}
+
+int gelu_fwd(int dtype, size_t n, const void* p, void* out, cudaStream_t s) {
+  if (n == 0) return PACI_OK;
+  const int V = dtype == PACI_BF16 ? 8 : 4;
+  if (n % V) return fail(PACI_EINVAL, "gelu: n not a multiple of %d", V);
+  const size_t nvec = n / V;
+  int blocks = (int)std::min<size_t>((nvec + 255) / 256, (size_t)num_sms() * 16);
+  if (dtype == PACI_BF16) PACI_LAUNCH(gelu_fwd_kernel<bf16>, blocks, 256, 0, s, nvec, (const bf16*)p, (bf16*)out);
+  else PACI_LAUNCH(gelu_fwd_kernel<float>, blocks, 256, 0, s, nvec, (const float*)p, (float*)out);
+  return PACI_OK;
+}
+
+// Column-slab kernel shared by gelu_bwd and colsum: thread owns one 16-byte column vector, the
+// block loops over rows (grid.y splits the rows), partial column sums stay in registers and end in
+// one global atomic per column per block.
+template <typename T, bool GELU>
+__global__ void __launch_bounds__(256) colslab_kernel(int rows, int cols, const T* __restrict__ a,
+                                                      const T* __restrict__ p, T* __restrict__ out,
+                                                      float* __restrict__ G) {
+  constexpr int V = Vec<T>::N;
+  const int c = (blockIdx.x * blockDim.x + threadIdx.x) * V;
+  if (c >= cols) return;
+  float acc[V];
+#pragma unroll
+  for (int j = 0; j < V; ++j) acc[j] = 0.f;
+  for (int r = blockIdx.y; r < rows; r += gridDim.y) {
+    const size_t off = (size_t)r * cols + c;
+    float v[V];
+    load_vec<T>(a + off, v);
+    if (GELU) {
+      float pv[V];
+      load_vec<T>(p + off, pv);
+#pragma unroll
+      for (int j = 0; j < V; ++j) v[j] *= dgelu_f(pv[j]);
+      store_vec<T>(out + off, v);
+#pragma unroll
+      for (int j = 0; j < V; ++j) v[j] = to_f(from_f<T>(v[j]));  // sum what was stored
+    }
+#pragma unroll
+    for (int j = 0; j < V; ++j) acc[j] += v[j];
+  }
+  if (G != nullptr) {
+#pragma unroll
+    for (int j = 0; j < V; ++j) atomicAdd(&G[c + j], acc[j]);
+  }
+}
+
+template <bool GELU>
+static int colslab(int dtype, int rows, int cols, const void* a, const void* p, void* out, float* G,
+                   cudaStream_t s) {
+  if (rows <= 0 || cols <= 0) return PACI_OK;
+  const int V = dtype == PACI_BF16 ? 8 : 4;
+  if (cols % V) return fail(PACI_EINVAL, "colslab: cols=%d not a multiple of %d", cols, V);
+  const int threads = 128;
+  const int gx = ceil_div(cols / V, threads);
+  int gy = std::max(1, num_sms() * 8 / gx);
+  if (gy > rows) gy = rows;
+  dim3 grid(gx, gy);
+  if (dtype == PACI_BF16)
+    PACI_LAUNCH((colslab_kernel<bf16, GELU>), grid, threads, 0, s, rows, cols, (const bf16*)a, (const bf16*)p,
+                (bf16*)out, G);
+  else
+    PACI_LAUNCH((colslab_kernel<float, GELU>), grid, threads, 0, s, rows, cols, (const float*)a,
+                (const float*)p, (float*)out, G);
+  return PACI_OK;
+}
+
+int gelu_bwd(int dtype, int rows, int cols, const void* dg, const void* p, void* dp, float* Gbias,
+             cudaStream_t s) {
+  return colslab<true>(dtype, rows, cols, dg, p, dp, Gbias, s);
+}
+int colsum(int dtype, int rows, int cols, const void* x, float* G, cudaStream_t s) {
+  return colslab<false>(dtype, rows, cols, x, nullptr, nullptr, G, s);
+}
+
+// =========================================================================== embedding
+template <typename T>
+__global__ void __launch_bounds__(256) embed_fwd_kernel(int M, int T_, int D, const int32_t* __restrict__ tok,
+                                                        const float* __restrict__ wte,
+                                                        const float* __restrict__ wpe, T* __restrict__ x) {
+  constexpr int V = Vec<T>::N;
+  const int nvec = D / V;
+  const size_t total = (size_t)M * nvec;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    const int row = (int)(i / nvec), c = (int)(i % nvec) * V;
+    const int id = tok[row], pos = row % T_;
+    float a[V], b[V];
+    load_f32<V>(wte + (size_t)id * D + c, a);
+    load_f32<V>(wpe + (size_t)pos * D + c, b);
+#pragma unroll
+    for (int j = 0; j < V; ++j) a[j] += b[j];
+    store_vec<T>(x + (size_t)row * D + c, a);
+  }
+}
+
+int embed_fwd(int dtype, int mu, int T_, int D, const int32_t* tok, const float* wte, const float* wpe, void* x,
+              cudaStream_t s) {
+  const int M = mu * T_;
+  const int V = dtype == PACI_BF16 ? 8 : 4;
+  if (D % V) return fail(PACI_EINVAL, "embed: D=%d", D);
+  const size_t total = (size_t)M * (D / V);
+  int blocks = (int)std::min<size_t>((total + 255) / 256, (size_t)num_sms() * 16);
+  if (dtype == PACI_BF16) PACI_LAUNCH(embed_fwd_kernel<bf16>, blocks, 256, 0, s, M, T_, D, tok, wte, wpe, (bf16*)x);
+  else PACI_LAUNCH(embed_fwd_kernel<float>, blocks, 256, 0, s, M, T_, D, tok, wte, wpe, (float*)x);
+  return PACI_OK;
+}
+
+// Gwte[tok] += dx (fp32 vector atomics: red.global.add.v4.f32), Gwpe[t] += sum_b dx[b,t].
+template <typename T>
+__global__ void __launch_bounds__(256) embed_bwd_wte_kernel(int M, int D, const int32_t* __restrict__ tok,
+                                                            const T* __restrict__ dx, float* __restrict__ Gwte) {
+  constexpr int V = Vec<T>::N;
+  const int nvec = D / V;
+  const size_t total = (size_t)M * nvec;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    const int row = (int)(i / nvec), c = (int)(i % nvec) * V;
+    float v[V];
+    load_vec<T>(dx + (size_t)row * D + c, v);
+    float* dst = Gwte + (size_t)tok[row] * D + c;
+#pragma unroll
+    for (int j = 0; j < V; j += 4)
+      asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + j), "f"(v[j]), "f"(v[j + 1]),
+                   "f"(v[j + 2]), "f"(v[j + 3])
+                   : "memory");
+  }
+}
+template <typename T>
+__global__ void __launch_bounds__(256) embed_bwd_wpe_kernel(int mu, int T_, int D, const T* __restrict__ dx,
+                                                            float* __restrict__ Gwpe) {
+  constexpr int V = Vec<T>::N;
+  const int nvec = D / V;
+  const size_t total = (size_t)T_ * nvec;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+    const int t = (int)(i / nvec), c = (int)(i % nvec) * V;
+    float acc[V];
+#pragma unroll
+    for (int j = 0; j < V; ++j) acc[j] = 0.f;
+    for (int b = 0; b < mu; ++b) {
+      float v[V];
+      load_vec<T>(dx + ((size_t)b * T_ + t) * D + c, v);
+#pragma unroll
+      for (int j = 0; j < V; ++j) acc[j] += v[j];
+    }
+    float* dst = Gwpe + (size_t)t * D + c;
+#pragma unroll
+    for (int j = 0; j < V; ++j) dst[j] += acc[j];
+  }
+}
+
+int embed_bwd(int dtype, int mu, int T_, int D, const int32_t* tok, const void* dx, float* Gwte, float* Gwpe,
+              cudaStream_t s) {
+  const int M = mu * T_;
+  const int V = dtype == PACI_BF16 ? 8 : 4;
+  if (D % V) return fail(PACI_EINVAL, "embed_bwd: D=%d", D);
+  const size_t t1 = (size_t)M * (D / V), t2 = (size_t)T_ * (D / V);
+  int b1 = (int)std::min<size_t>((t1 + 255) / 256, (size_t)num_sms() * 16);
+  int b2 = (int)std::min<size_t>((t2 + 255) / 256, (size_t)num_sms() * 16);
+  if (dtype == PACI_BF16) {
+    PACI_LAUNCH(embed_bwd_wte_kernel<bf16>, b1, 256, 0, s, M, D, tok, (const bf16*)dx, Gwte);
+    PACI_LAUNCH(embed_bwd_wpe_kernel<bf16>, b2, 256, 0, s, mu, T_, D, (const bf16*)dx, Gwpe);
+  } else {
+    PACI_LAUNCH(embed_bwd_wte_kernel<float>, b1, 256, 0, s, M, D, tok, (const float*)dx, Gwte);
+    PACI_LAUNCH(embed_bwd_wpe_kernel<float>, b2, 256, 0, s, mu, T_, D, (const float*)dx, Gwpe);
+  }
+  return PACI_OK;
+}
+
+// =========================================================================== softmax cross-entropy
+// One block per token row: pass 1 reads the row (online max / sum of exp), pass 2 re-reads it (L2
+// hit: a row is <= 100 KB) and overwrites it with dz = (softmax - onehot) / rows.  Padding columns
+// [V, ldz) are written as 0 so that the following GEMMs can contract over ldz.
+template <typename T> __device__ __forceinline__ float exp_t(float x);
+template <> __device__ __forceinline__ float exp_t<float>(float x) { return expf(x); }     // 1e-5 parity mode
+template <> __device__ __forceinline__ float exp_t<bf16>(float x) { return __expf(x); }
+
+template <typename T>
+__global__ void __launch_bounds__(512) softmax_ce_kernel(int rows, int V_, int ldz, T* __restrict__ z,
+                                                         const int32_t* __restrict__ tgt,
+                                                         float* __restrict__ loss) {
+  constexpr int V = Vec<T>::N;
+  __shared__ float red_m[16], red_s[16];
+  __shared__ float sh_max, sh_sum;
+  const int row = blockIdx.x;
+  T* zr = z + (size_t)row * ldz;
+  const int nvec = ldz / V;
+  float mx = -INFINITY, sum = 0.f;
+  for (int i = threadIdx.x; i < nvec; i += blockDim.x) {
+    float v[V];
+    load_vec<T>(zr + (size_t)i * V, v);
+    float lm = -INFINITY;
+#pragma unroll
+    for (int j = 0; j < V; ++j)
+      if (i * V + j < V_) lm = fmaxf(lm, v[j]);
+    if (lm > mx) {
+      sum *= exp_t<T>(mx - lm);
+      mx = lm;
+    }
+#pragma unroll
+    for (int j = 0; j < V; ++j)
+      if (i * V + j < V_) sum += exp_t<T>(v[j] - mx);
+  }
+  // block reduce (max, sum) pairs
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  float wm = warp_max(mx);
+  float ws = warp_sum(mx == -INFINITY ? 0.f : sum * exp_t<T>(mx - wm));
+  if (lane == 0) { red_m[w] = wm; red_s[w] = ws; }
+  __syncthreads();
+  if (w == 0) {
+    const int nw = blockDim.x >> 5;
+    float m2 = lane < nw ? red_m[lane] : -INFINITY;
+    float s2 = lane < nw ? red_s[lane] : 0.f;
+    const float bm = warp_max(m2);
+    const float bs = warp_sum(m2 == -INFINITY ? 0.f : s2 * exp_t<T>(m2 - bm));
+    if (lane == 0) { sh_max = bm; sh_sum = bs; }
+  }
+  __syncthreads();
+  const float bm = sh_max, inv = 1.f / sh_sum, scale = 1.f / (float)rows;
+  const int t = tgt[row];
+  if (threadIdx.x == 0) {
+    const float zt = to_f(zr[t]);
+    atomicAdd(loss, (logf(sh_sum) + bm - zt) * scale);
+  }
+  __syncthreads();  // zr[t] read before anyone overwrites it
+  for (int i = threadIdx.x; i < nvec; i += blockDim.x) {
+    float v[V];
+    load_vec<T>(zr + (size_t)i * V, v);
+#pragma unroll
+    for (int j = 0; j < V; ++j) {
+      const int c = i * V + j;
+      float p = c < V_ ? exp_t<T>(v[j] - bm) * inv : 0.f;
+      if (c == t) p -= 1.f;
+      v[j] = p * scale;
+    }
+    store_vec<T>(zr + (size_t)i * V, v);
+  }
+}
+
+int softmax_ce(int dtype, int rows, int V_, int ldz, void* z, const int32_t* tgt, float* loss, cudaStream_t s) {
+  const int V = dtype == PACI_BF16 ? 8 : 4;
+  if (ldz % V || ldz < V_) return fail(PACI_EINVAL, "softmax_ce: ldz=%d V=%d", ldz, V_);
+  if (dtype == PACI_BF16) PACI_LAUNCH(softmax_ce_kernel<bf16>, rows, 512, 0, s, rows, V_, ldz, (bf16*)z, tgt, loss);
+  else PACI_LAUNCH(softmax_ce_kernel<float>, rows, 512, 0, s, rows, V_, ldz, (float*)z, tgt, loss);
+  return PACI_OK;
+}
+
+// =========================================================================== fused multi-tensor AdamW
+// The stage's parameters live in ONE flat fp32 arena laid out [decayed tensors | non-decayed tensors],
+// so a single launch covers every tensor (row a20): 34 B/param in bf16 mode (read w,m,v,G; write
+// w,m,v,G=0 and the bf16 shadow).  Thread 0 bumps the device version word (Alg. 1 line 17).
+__global__ void __launch_bounds__(256) adamw_kernel(size_t n4, size_t n4_decay, float4* __restrict__ w,
+                                                    float4* __restrict__ m, float4* __restrict__ v,
+                                                    float4* __restrict__ G, uint2* __restrict__ shadow,
+                                                    float inv_k, float lr, float beta1, float beta2, float eps,
+                                                    float decay_mul, float inv_bc1, float inv_bc2,
+                                                    int64_t* version_word) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
+    float4 W = w[i], Mv = m[i], Vv = v[i], Gv = G[i];
+    const float dm = i < n4_decay ? decay_mul : 1.f;
+    float* wp = reinterpret_cast<float*>(&W);
+    float* mp = reinterpret_cast<float*>(&Mv);
+    float* vp = reinterpret_cast<float*>(&Vv);
+    const float* gp = reinterpret_cast<const float*>(&Gv);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const float g = gp[j] * inv_k;
+      float th = wp[j] * dm;
+      mp[j] = beta1 * mp[j] + (1.f - beta1) * g;
+      vp[j] = beta2 * vp[j] + (1.f - beta2) * g * g;
+      th -= lr * (mp[j] * inv_bc1) / (sqrtf(vp[j] * inv_bc2) + eps);
+      wp[j] = th;
+    }
+    w[i] = W; m[i] = Mv; v[i] = Vv;
+    G[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (shadow != nullptr) {
+      __nv_bfloat162 lo = __floats2bfloat162_rn(W.x, W.y), hi = __floats2bfloat162_rn(W.z, W.w);
+      uint2 o;
+      o.x = *reinterpret_cast<uint32_t*>(&lo);
+      o.y = *reinterpret_cast<uint32_t*>(&hi);
+      shadow[i] = o;
+    }
+  }
+  if (version_word != nullptr && blockIdx.x == 0 && threadIdx.x == 0) *version_word += 1;
+}
+
+int adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float* G, void* shadow, int k, int64_t t,
+          float lr, float beta1, float beta2, float eps, float wd, int64_t* version_word, cudaStream_t s) {
+  if (n % 4 || n_decay % 4) return fail(PACI_EINVAL, "adamw: n=%zu n_decay=%zu must be multiples of 4", n, n_decay);
+  const double bc1 = 1.0 - std::pow((double)beta1, (double)t), bc2 = 1.0 - std::pow((double)beta2, (double)t);
+  const size_t n4 = n / 4;
+  int blocks = (int)std::min<size_t>(std::max<size_t>((n4 + 255) / 256, 1), (size_t)num_sms() * 8);
+  PACI_LAUNCH(adamw_kernel, blocks, 256, 0, s, n4, n_decay / 4, (float4*)w, (float4*)m, (float4*)v, (float4*)G,
+              (uint2*)shadow, 1.f / (float)k, lr, beta1, beta2, eps, 1.f - lr * wd, (float)(1.0 / bc1),
+              (float)(1.0 / bc2), version_word);
+  return PACI_OK;
+}
+
+__global__ void cast_shadow_kernel(size_t n, const float* __restrict__ w, bf16* __restrict__ sh) {
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    sh[i] = __float2bfloat16_rn(w[i]);
+}
+int cast_shadow(size_t n, const float* w, void* shadow, cudaStream_t s) {
+  if (n == 0) return PACI_OK;
+  int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)num_sms() * 8);
+  PACI_LAUNCH(cast_shadow_kernel, blocks, 256, 0, s, n, w, (bf16*)shadow);
+  return PACI_OK;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) add_vec_kernel(size_t nvec, const T* __restrict__ a, const T* __restrict__ b,
+                                                      T* __restrict__ out) {
+  constexpr int V = Vec<T>::N;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    float x[V];
+    load_vec<T>(a + i * V, x);
+    if (b != nullptr) {
+      float y[V];
+      load_vec<T>(b + i * V, y);
+#pragma unroll
+      for (int j = 0; j < V; ++j) x[j] += y[j];
+    }
+    store_vec<T>(out + i * V, x);
+  }
+}
+int add_vec(int dtype, size_t n, const void* a, const void* b, void* out, cudaStream_t s) {
+  if (n == 0) return PACI_OK;
+  const int V = dtype == PACI_BF16 ? 8 : 4;
+  if (n % V) return fail(PACI_EINVAL, "add: n not a multiple of %d", V);
+  const size_t nvec = n / V;
+  int blocks = (int)std::min<size_t>((nvec + 255) / 256, (size_t)num_sms() * 16);
+  if (dtype == PACI_BF16)
+    PACI_LAUNCH(add_vec_kernel<bf16>, blocks, 256, 0, s, nvec, (const bf16*)a, (const bf16*)b, (bf16*)out);
+  else
+    PACI_LAUNCH(add_vec_kernel<float>, blocks, 256, 0, s, nvec, (const float*)a, (const float*)b, (float*)out);
+  return PACI_OK;
+}
+
+__global__ void stamp_kernel(const int64_t* version_word, int64_t* dst) { *dst = *version_word; }
+int stamp_version(const int64_t* version_word, int64_t* dst, cudaStream_t s) {
+  PACI_LAUNCH(stamp_kernel, 1, 1, 0, s, version_word, dst);
+  return PACI_OK;
+}
+
+__global__ void split_tokens_kernel(int mu, int T_, const int32_t* __restrict__ src, int32_t* __restrict__ inp,
+                                    int32_t* __restrict__ tgt) {
+  const int n = mu * T_;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const int b = i / T_, t = i % T_;
+    inp[i] = src[(size_t)b * (T_ + 1) + t];
+    tgt[i] = src[(size_t)b * (T_ + 1) + t + 1];
+  }
+}
+int split_tokens(int mu, int T_, const int32_t* tok_tp1, int32_t* inp, int32_t* tgt, cudaStream_t s) {
+  PACI_LAUNCH(split_tokens_kernel, ceil_div(mu * T_, 256), 256, 0, s, mu, T_, tok_tp1, inp, tgt);
+  return PACI_OK;
+}
+
+}  // namespace paci

@@ -1,0 +1,120 @@
+// ops.cu -- backend dispatch (fp32 -> FFMA kernels, bf16 -> tcgen05 / tensor-core kernels) and the
+// op-level C-ABI entry points used by the kernel parity tests and the per-kernel roofline benches.
+#include <cstdlib>
+#include <cstring>
+
+#include "common.cuh"
+
+namespace paci {
+
+static bool env_is(const char* name, const char* val) {
+  const char* e = std::getenv(name);
+  return e != nullptr && std::strcmp(e, val) == 0;
+}
+
+// PACI_GEMM=simt / PACI_ATTN=simt force the CUDA-core kernels in bf16 mode: a debugging aid to
+// bisect a parity failure, reported by paci_gemm_backend_is_tcgen05(); never selected silently.
+bool gemm_backend_tcgen05() {
+  static const bool simt = env_is("PACI_GEMM", "simt");
+  return !simt;
+}
+static bool attn_backend_tensor() {
+  static const bool simt = env_is("PACI_ATTN", "simt");
+  return !simt;
+}
+
+int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
+         const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s) {
+  if (dtype == PACI_BF16 && gemm_backend_tcgen05())
+    return gemm_tc(layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, s);
+  return gemm_simt(dtype, layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, s);
+}
+
+int attention_fwd_mma(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
+int attention_bwd_mma(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
+                      void* dqkv, float* scratch, cudaStream_t s);
+size_t attention_bwd_mma_scratch_bytes(int mu, int T, int H);
+
+int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse, cudaStream_t s) {
+  if (dtype == PACI_BF16 && attn_backend_tensor()) {
+    if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
+    return attention_fwd_mma(mu, T, H, qkv, o, lse, s);
+  }
+  return attention_fwd_simt(dtype, mu, T, H, dh, qkv, o, lse, s);
+}
+
+int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv, const void* o,
+                  const float* lse, void* dqkv, float* scratch, cudaStream_t s) {
+  if (dtype == PACI_BF16 && attn_backend_tensor()) {
+    if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
+    return attention_bwd_mma(mu, T, H, dout, qkv, o, lse, dqkv, scratch, s);
+  }
+  return attention_bwd_simt(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, s);
+}
+
+size_t attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh) {
+  size_t simt = (size_t)mu * H * T * sizeof(float);
+  if (dtype == PACI_BF16 && dh == 64) return std::max(simt, attention_bwd_mma_scratch_bytes(mu, T, H));
+  return simt;
+}
+
+}  // namespace paci
+
+using namespace paci;
+
+extern "C" {
+
+int paci_op_gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
+                 const float* bias, void* C, int ldc, int out_f32_accum, void* stream) {
+  return gemm(dtype, layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, (cudaStream_t)stream);
+}
+int paci_op_layernorm_fwd(int dtype, int rows, int D, const void* x, const void* res, const float* g,
+                          const float* b, void* xsum, void* y, float* mean, float* rstd, void* stream) {
+  return ln_fwd(dtype, rows, D, x, res, g, b, xsum, y, mean, rstd, (cudaStream_t)stream);
+}
+int paci_op_layernorm_bwd(int dtype, int rows, int D, const void* dy, const void* x, const float* mean,
+                          const float* rstd, const float* g, const void* dres, void* dx, float* Gg, float* Gb,
+                          float* Gcol, void* stream) {
+  return ln_bwd(dtype, rows, D, dy, x, mean, rstd, g, dres, dx, Gg, Gb, Gcol, (cudaStream_t)stream);
+}
+int paci_op_gelu_fwd(int dtype, size_t n, const void* p, void* out, void* stream) {
+  return gelu_fwd(dtype, n, p, out, (cudaStream_t)stream);
+}
+int paci_op_gelu_bwd(int dtype, int rows, int cols, const void* dg, const void* p, void* dp, float* Gbias,
+                     void* stream) {
+  return gelu_bwd(dtype, rows, cols, dg, p, dp, Gbias, (cudaStream_t)stream);
+}
+int paci_op_colsum(int dtype, int rows, int cols, const void* x, float* G, void* stream) {
+  return colsum(dtype, rows, cols, x, G, (cudaStream_t)stream);
+}
+int paci_op_attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,
+                          void* stream) {
+  return attention_fwd(dtype, mu, T, H, dh, qkv, o, lse, (cudaStream_t)stream);
+}
+int paci_op_attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
+                          const void* o, const float* lse, void* dqkv, float* scratch, void* stream) {
+  return attention_bwd(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, (cudaStream_t)stream);
+}
+size_t paci_op_attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh) {
+  return attention_bwd_scratch_bytes(dtype, mu, T, H, dh);
+}
+int paci_op_embed_fwd(int dtype, int mu, int T, int D, const int32_t* tok, const float* wte, const float* wpe,
+                      void* x, void* stream) {
+  return embed_fwd(dtype, mu, T, D, tok, wte, wpe, x, (cudaStream_t)stream);
+}
+int paci_op_embed_bwd(int dtype, int mu, int T, int D, const int32_t* tok, const void* dx, float* Gwte,
+                      float* Gwpe, void* stream) {
+  return embed_bwd(dtype, mu, T, D, tok, dx, Gwte, Gwpe, (cudaStream_t)stream);
+}
+int paci_op_softmax_ce(int dtype, int rows, int V, int ldz, void* z, const int32_t* tgt, float* loss,
+                       void* stream) {
+  return softmax_ce(dtype, rows, V, ldz, z, tgt, loss, (cudaStream_t)stream);
+}
+int paci_op_adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float* G, void* shadow_bf16, int k,
+                  int64_t t, float lr, float beta1, float beta2, float eps, float weight_decay,
+                  int64_t* version_word, void* stream) {
+  return adamw(n, n_decay, w, m, v, G, shadow_bf16, k, t, lr, beta1, beta2, eps, weight_decay, version_word,
+               (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,92 @@
+"""-m gpu: the schedule driver (S emulated stages on one GPU) vs the oracle pipeline: exact integer
+agreement on crossed-update counts and versions; losses, accumulators and weights within tolerance."""
+import numpy as np
+import pytest
+import torch
+
+import synth
+from oracle import model, pipeline as opipe
+from paper_2606_07881_b200 import binding as pb
+from gpu_util import TOL, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+
+def _build(dtype, S, L, D, H, T, mu, V, k, seed=1234):
+    specs = [model.StageSpec(s, S, L, D, H, T, mu, V) for s in range(S)]
+    params = [synth.stage_params(seed, s, S, L, D, V, T, perturbed=True) for s in range(S)]
+    stages = []
+    for s in range(S):
+        st = pb.Stage(pb.make_config(s, S, L, D, H, T, mu, k, V, dtype))
+        st.load_params(params[s])
+        stages.append(st)
+    return specs, params, stages
+
+
+def _compare(out, ref, stages, dtype, n, loss_tol):
+    assert out["delta"].tolist() == ref["delta"]                 # exact (Eq. 8)
+    assert out["version"].tolist() == ref["version"]             # exact
+    assert out["max_q"].tolist() == ref["sim"]["max_q"]
+    assert np.max(np.abs(out["loss"] - np.array(ref["losses"])) / np.array(ref["losses"])) < loss_tol
+    for s, st in enumerate(stages):
+        for name, th in ref["opt"][s].theta.items():
+            assert rel_l2(st.read(name), th) < TOL[dtype], (s, name)
+
+
+def test_cfg1_tiny_fp32_full_schedule():
+    """BASELINE.json configs[0] at full size: 2 stages x 1 block, k=4, 16 micro-batches, lr 1e-3."""
+    V, D, H, T, mu, S, L, k, n = 256, 64, 4, 32, 2, 2, 1, 4, 16
+    specs, params, stages = _build(pb.FP32, S, L, D, H, T, mu, V, k)
+    tok = synth.tokens(1234, n, mu, T, V, "uniform")
+    ref = opipe.run_pipeline(specs, params, tok, k, 1e-3)
+    pipe = pb.Pipeline(stages)
+    out = pipe.run(torch.from_numpy(tok).cuda(), 1e-3)
+    assert ref["delta"][0] == [1 if m in (4, 8, 12) else 0 for m in range(16)]
+    _compare(out, ref, stages, pb.FP32, n, 1e-5)
+    assert out["n_slots"] == ref["sim"]["makespan"] == 2 * n + 2 * (S - 1)
+    assert out["n_launches"] > 0
+    for m in range(n):
+        vF, vB = stages[0].device_stamps(m)
+        assert vB - vF == ref["delta"][0][m]                      # device-side proof of host Delta
+
+
+def test_host_token_path_equals_resident_path():
+    V, D, H, T, mu, S, L, k, n = 256, 64, 4, 32, 2, 2, 1, 2, 4
+    tok = synth.tokens(7, n, mu, T, V, "uniform")
+    res = []
+    for host_side in (False, True):
+        _, _, stages = _build(pb.FP32, S, L, D, H, T, mu, V, k)
+        out = pb.Pipeline(stages).run(tok if host_side else torch.from_numpy(tok).cuda(), 1e-3)
+        res.append((out["loss"].copy(), stages[0].read("wte")))
+    assert np.allclose(res[0][0], res[1][0], rtol=1e-6) and np.allclose(res[0][1], res[1][1], rtol=1e-5, atol=1e-7)
+
+
+@pytest.mark.parametrize("S,k,n", [(3, 2, 8), (4, 1, 6), (1, 3, 6)])
+def test_fp32_deeper_pipelines_and_k_sweep(S, k, n):
+    V, D, H, T, mu, L = 128, 32, 2, 16, 2, 1
+    specs, params, stages = _build(pb.FP32, S, L, D, H, T, mu, V, k, seed=5)
+    tok = synth.tokens(5, n, mu, T, V, "zipf")
+    ref = opipe.run_pipeline(specs, params, tok, k, 2e-3)
+    out = pb.Pipeline(stages).run(torch.from_numpy(tok).cuda(), 2e-3)
+    _compare(out, ref, stages, pb.FP32, n, 2e-5)
+
+
+def test_flush_mode_matches_oracle_and_never_crosses():
+    V, D, H, T, mu, S, L, m_f, n = 128, 32, 2, 16, 2, 3, 1, 2, 6
+    specs, params, stages = _build(pb.FP32, S, L, D, H, T, mu, V, m_f, seed=6)
+    tok = synth.tokens(6, n, mu, T, V, "zipf")
+    ref = opipe.run_pipeline(specs, params, tok, None, 2e-3, mode="flush", m_f=m_f)
+    out = pb.Pipeline(stages).run(torch.from_numpy(tok).cuda(), 2e-3, mode=pb.MODE_FLUSH)
+    assert np.all(out["delta"] == 0)
+    _compare(out, ref, stages, pb.FP32, n, 2e-5)
+    assert out["n_slots"] == ref["sim"]["makespan"]
+
+
+def test_bf16_pipeline_small():
+    """bf16 mode, 3 stages: counts exact, loss / weights within the bf16 gates after two updates."""
+    V, D, H, T, mu, S, L, k, n = 1000, 128, 2, 64, 2, 3, 1, 2, 4
+    specs, params, stages = _build(pb.BF16, S, L, D, H, T, mu, V, k, seed=9)
+    tok = synth.tokens(9, n, mu, T, V, "zipf")
+    ref = opipe.run_pipeline(specs, params, tok, k, 3e-4)
+    out = pb.Pipeline(stages).run(torch.from_numpy(tok).cuda(), 3e-4)
+    _compare(out, ref, stages, pb.BF16, n, 5e-3)
