@@ -246,7 +246,7 @@ static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float*
                 rstd, g, (const T*)dres, (T*)dx, Gg, Gb, Gcol);                                         \
     break;
   switch (nv) {
-    LNB_CASE(1) LNB_CASE(2) LNB_CASE(3) LNB_CASE(4) LNB_CASE(5) LNB_CASE(6)
+    LNB_CASE(1) LNB_CASE(2) LNB_CASE(3) LNB_CASE(4) LNB_CASE(5) LNB_CASE(6) LNB_CASE(7) LNB_CASE(8)
     default: return fail(PACI_EINVAL, "layernorm_bwd: D=%d too large", D);
   }
 #undef LNB_CASE

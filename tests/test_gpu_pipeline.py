@@ -23,14 +23,31 @@ def _build(dtype, S, L, D, H, T, mu, V, k, seed=1234):
     return specs, params, stages
 
 
-def _compare(out, ref, stages, dtype, n, loss_tol):
+# Weights after AdamW steps: on the first steps the update is ~ lr*sign(g) (SURVEY 8(c) note), so an
+# element whose gradient is within rounding of zero can flip sign and move by 2*lr.  With per-tensor
+# gradient error e (1e-5 fp32) a fraction ~e of the elements flips: rel-L2 ~ sqrt(e)*2*lr/rms(w) ~ 3e-4
+# at lr 1e-3, rms 0.02.  Gate: 1e-3 in fp32 mode (derived), 2e-2 in bf16 mode (BASELINE.json).
+WTOL = {pb.FP32: 1e-3, pb.BF16: 2e-2}
+
+
+def _compare(out, ref, stages, dtype, n, loss_tol, lr_bound=2e-3):
     assert out["delta"].tolist() == ref["delta"]                 # exact (Eq. 8)
     assert out["version"].tolist() == ref["version"]             # exact
     assert out["max_q"].tolist() == ref["sim"]["max_q"]
     assert np.max(np.abs(out["loss"] - np.array(ref["losses"])) / np.array(ref["losses"])) < loss_tol
     for s, st in enumerate(stages):
         for name, th in ref["opt"][s].theta.items():
-            assert rel_l2(st.read(name), th) < TOL[dtype], (s, name)
+            got, th = st.read(name), th.reshape(-1)
+            if name.endswith("attn.bqkv"):     # key bias: zero gradient, Adam amplifies rounding noise to <= lr
+                D = th.size // 3
+                assert np.max(np.abs(got[D:2 * D] - th[D:2 * D])) <= lr_bound * out["version"][s] * 1.001
+                got, th = np.delete(got, np.r_[D:2 * D]), np.delete(th, np.r_[D:2 * D])
+            assert rel_l2(got, th) < WTOL[dtype], (s, name)
+            G = ref["opt"][s].G[name]                            # tail window (n % k backwards) stays in G
+            if np.any(G):
+                assert rel_l2(st.read(name, pb.GRAD_ACCUM), G) < 4 * TOL[dtype], (s, name)
+            else:
+                assert np.count_nonzero(st.read(name, pb.GRAD_ACCUM)) == 0
 
 
 def test_cfg1_tiny_fp32_full_schedule():
@@ -61,7 +78,7 @@ def test_host_token_path_equals_resident_path():
     assert np.allclose(res[0][0], res[1][0], rtol=1e-6) and np.allclose(res[0][1], res[1][1], rtol=1e-5, atol=1e-7)
 
 
-@pytest.mark.parametrize("S,k,n", [(3, 2, 8), (4, 1, 6), (1, 3, 6)])
+@pytest.mark.parametrize("S,k,n", [(3, 2, 9), (4, 1, 6), (1, 3, 7), (2, 4, 6)])
 def test_fp32_deeper_pipelines_and_k_sweep(S, k, n):
     V, D, H, T, mu, L = 128, 32, 2, 16, 2, 1
     specs, params, stages = _build(pb.FP32, S, L, D, H, T, mu, V, k, seed=5)

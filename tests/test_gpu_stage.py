@@ -94,7 +94,8 @@ def test_drift_case_stale_activations_current_weights(dtype, D, H, T, V):
     _, stash1 = model.stage_forward(spec, opt.theta, b[2])
     _, g0 = model.stage_backward(spec, opt.theta, stash0, a[3])
     opt.accumulate(g0)
-    assert opt.maybe_step(1e-2)
+    lr = 1e-2 if dtype == pb.FP32 else 1e-3   # bf16: keep Adam's sign-flip noise (~sqrt(f)*2lr/rms) small
+    assert opt.maybe_step(lr)
     ref_din, g1 = model.stage_backward(spec, opt.theta, stash1, b[3])      # current weights, old stash
     _, g1_consistent = model.stage_backward(spec, {n: np.asarray(p, np.float64) for n, p in params.items()},
                                             stash1, b[3])
@@ -112,7 +113,7 @@ def test_drift_case_stale_activations_current_weights(dtype, D, H, T, V):
     with pytest.raises(pb.PaciError) as e:                                  # c == k: update pending
         st.backward(1, dev(b[3], dtype), torch.empty_like(k0[2]))
     assert e.value.code == pb.ESTATE
-    assert st.maybe_step(1e-2) == 1 and st.version == 1 and st.maybe_step(1e-2) == 0
+    assert st.maybe_step(lr) == 1 and st.version == 1 and st.maybe_step(lr) == 0
     din1 = torch.empty_like(k0[2])
     st.backward(1, dev(b[3], dtype), din1)
     torch.cuda.synchronize()
@@ -152,7 +153,15 @@ def test_window_of_k_then_update_matches_oracle(dtype):
     assert st.version == 1 and st.window_count == 0
     for name in opt.theta:
         got = st.read(name)
-        assert rel_l2(got, opt.theta[name]) < TOL[dtype], name                  # weights after one step
+        ref = opt.theta[name].reshape(-1)
+        if name.endswith("attn.bqkv"):
+            # The key bias has an identically ZERO gradient (softmax is invariant to a constant added to
+            # every key: sum_j ds_ij = 0), so what reaches AdamW is rounding noise, which Adam normalises
+            # to a step of up to +-lr.  Compare q and v parts; bound the k part by lr.
+            kpart = slice(D, 2 * D)
+            assert np.max(np.abs(got[kpart] - ref[kpart])) <= 1e-3 * 1.001
+            got, ref = np.delete(got, np.r_[kpart]), np.delete(ref, np.r_[kpart])
+        assert rel_l2(got, ref) < (1e-3 if dtype == pb.FP32 else 2e-2), name               # after one step
         assert np.count_nonzero(st.read(name, pb.GRAD_ACCUM)) == 0            # G reset
     # weight DELTA: first step ~ lr*sign(g); bf16 can flip the sign of near-zero gradients
     d_got = st.read("h.0.mlp.w1") - theta0["h.0.mlp.w1"].reshape(-1)

@@ -9,7 +9,6 @@ import torch.nn.functional as F
 import synth
 from oracle import model
 
-torch.set_default_dtype(torch.float64)
 
 
 def _spec(stage_index=0, n_stages=1, n_layers=1, D=16, H=4, T=8, mu=2, V=32):

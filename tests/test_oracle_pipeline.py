@@ -9,7 +9,6 @@ import synth
 from oracle import model, pipeline
 from test_oracle_layers import _torch_stage
 
-torch.set_default_dtype(torch.float64)
 
 CFG = dict(D=32, H=4, T=16, mu=2, V=64)
 
