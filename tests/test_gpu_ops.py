@@ -191,10 +191,13 @@ def test_gemm_layouts(dtype, layout, M, N, K):
     A = rng.standard_normal((M, K)); B = rng.standard_normal((N, K)); bias = rng.standard_normal(N)
     Ar, Br = rounded(A, dtype), rounded(B, dtype)
     ref = Ar @ Br.T
-    Ad = dev(A if layout != 2 else A.T, dtype)          # TN: A stored [K, M]
-    Bd = dev(B if layout == 0 else B.T, dtype)          # NN/TN: B stored [K, N]
-    lda = K if layout != 2 else M
-    ldb = K if layout == 0 else N
+    def padded(a):                                      # row stride rounded up to 8 elements (16 B in bf16),
+        ld = (a.shape[1] + 7) // 8 * 8                  # with garbage in the padding: ld != extent is exercised
+        buf = np.full((a.shape[0], ld), 9.0)
+        buf[:, :a.shape[1]] = a
+        return dev(buf, dtype), ld
+    Ad, lda = padded(A if layout != 2 else A.T)         # TN: A stored [K, M]
+    Bd, ldb = padded(B if layout == 0 else B.T)         # NN/TN: B stored [K, N]
     Cd = torch.empty(M, N, device="cuda", dtype=DT[dtype])
     ck(lib.paci_op_gemm(dtype, layout, M, N, K, Ad.data_ptr(), lda, Bd.data_ptr(), ldb, f32(bias).data_ptr(),
                         Cd.data_ptr(), N, 0, S0))
