@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py -- the PACI stage-step benchmark (contract in DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config medium] [--impl reference]
+
+One STEP = one global batch (n_micro micro-batches) pushed through the S emulated stages of the
+asynchronous 1F1B pipeline on one GPU by `paci_pipeline_run`: every row of SURVEY.md 8(a) runs --
+embedding, the block stacks forward and backward, LM head + cross-entropy, wgrad accumulation into
+fp32 in the GEMM epilogue, one fused AdamW per stage every k micro-batches, version / crossed-update
+bookkeeping.  Metric (BASELINE.json): tokens/s per PACI stage step = stage steps x tokens per
+micro-batch / time, i.e. S * n_micro * mu * T / t_step (mean over the S stages of the pipeline; the
+whole-pipeline tokens/s is the same number / S and is printed as `pipeline_tokens_per_s`).
+
+Prints ONE JSON line on rank 0.  N > 1 (torchrun): N independent replicas, no data-path collective
+("replicas only"); barrier + max-over-ranks timing.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+# BASELINE.json `configs`, in order.  n_micro = micro-batches per step (one global batch).
+CONFIGS = {
+    "tiny":    dict(idx=0, V=256,   D=64,   H=4,  T=32,   S=2, L=1, mu=2,  k=4, n_micro=16, dtype="fp32",
+                    dist="uniform", lr=1e-3),
+    "small":   dict(idx=1, V=50257, D=768,  H=12, T=1024, S=4, L=3, mu=8,  k=4, n_micro=16, dtype="bf16",
+                    dist="zipf", lr=3e-4),
+    "medium":  dict(idx=2, V=50257, D=1024, H=16, T=1024, S=4, L=6, mu=8,  k=4, n_micro=16, dtype="bf16",
+                    dist="zipf", lr=3e-4),
+    "medium8": dict(idx=3, V=50257, D=1024, H=16, T=1024, S=8, L=3, mu=8,  k=4, n_micro=32, dtype="bf16",
+                    dist="zipf", lr=3e-4),
+    "large":   dict(idx=4, V=50257, D=1280, H=20, T=1024, S=1, L=9, mu=16, k=8, n_micro=16, dtype="bf16",
+                    dist="zipf", lr=3e-4),
+}
+METRIC = "tokens/s per PACI stage step (GPT-2 Medium, bf16)"
+UNIT = "tokens/s"
+SEED = 1   # timing seed; parity uses 1234
+
+
+def workload_name(name, c):
+    return (f"configs[{c['idx']}] {name}: V={c['V']} D={c['D']} H={c['H']} T={c['T']} "
+            f"{c['S']} emulated stages x {c['L']} pre-LN blocks, micro-batch {c['mu']}, k={c['k']}, "
+            f"{c['n_micro']} micro-batches per step, {c['dtype']} compute / fp32 master+m+v+G, "
+            f"{c['dist']} tokens, N(0,0.02) weights")
+
+
+# ------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 9:
+                continue
+            try:
+                sm.append(float(parts[1])); mx.append(float(parts[2])); pw.append(float(parts[3]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        os.unlink(self.f.name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        busy = sorted(s for s, p in zip(sm, pw) if p > 0.5 * max(pw)) or sorted(sm)
+        return {"sm_mhz": busy[len(busy) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------ peaks
+def measured_peaks():
+    """MEASURED_PEAKS.json (driver-written) or the profiling guide's stated fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return dict(hbm=d["hbm_gbs"], tf_burst=d["bf16_tflops"],
+                    tf_sustained=d.get("bf16_tflops_sustained", d["bf16_tflops"]), source="measured")
+    return dict(hbm=6650.0, tf_burst=1590.0, tf_sustained=1400.0, source="fallback")
+
+
+def ncu_traffic(kernel_key):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+    p = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            parts = [x.strip() for x in line.split(",")]
+            if parts and parts[0] == kernel_key and len(parts) >= 3:
+                try:
+                    return float(parts[1]) + float(parts[2])
+                except ValueError:
+                    return None
+    return None
+
+
+# ------------------------------------------------------------------------------------ CPU oracle leg
+def oracle_sample(c, steps, warmup):
+    """Times the fp64 oracle AS IT STANDS on the host cores, on a bounded sample of the workload: one
+    PACI stage step (F, B with G += g, and the AdamW update divided by k as in the workload) of ONE
+    stage at full width and depth (L blocks, D, H, T, V), with micro-batch 1.  The stage is the
+    interior stage s=1 when S >= 3 (the stage kind SURVEY.md 8(d) defines the metric on), else stage 0.
+    Returns (tokens/s per stage step, info)."""
+    import synth
+    from oracle import model
+    from oracle.adamw import StageOptimizer
+    S, L, D, H, T, V, k = c["S"], c["L"], c["D"], c["H"], c["T"], c["V"], c["k"]
+    mu = 1
+    s = 1 if S >= 3 else 0
+    spec = model.StageSpec(s, S, L, D, H, T, mu, V)
+    opt = StageOptimizer(synth.stage_params(SEED, s, S, L, D, V, T), 1)
+    tok = synth.tokens(SEED, steps + warmup, mu, T, V, c["dist"])
+    rng = np.random.default_rng(SEED)
+    per_step = []
+    for it in range(steps + warmup):
+        inp = tok[it, :, :-1].astype(np.int64) if spec.has_embedding else rng.standard_normal((mu, T, D))
+        tgt = tok[it, :, 1:].astype(np.int64) if spec.has_head else None
+        dout = None if spec.has_head else rng.standard_normal((mu, T, D)) * 1e-3
+        t0 = time.perf_counter()
+        _, stash = model.stage_forward(spec, opt.theta, inp, tgt)
+        _, grads = model.stage_backward(spec, opt.theta, stash, dout)
+        opt.accumulate(grads)
+        t_fb = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        assert opt.maybe_step(c["lr"])
+        t_u = time.perf_counter() - t0
+        per_step.append(t_fb + t_u / k)
+    timed = per_step[warmup:]
+    t = sum(timed) / len(timed)
+    host = len(os.sched_getaffinity(0))
+    try:
+        from threadpoolctl import threadpool_info
+        threads = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
+    except Exception:
+        threads = host
+    kind = "interior" if 0 < s < S - 1 else ("first" if S > 1 else "only")
+    info = dict(cores=min(threads, host), host_cores=host, s_per_step=t,
+                sample=(f"fp64 numpy oracle: one stage step of the {kind} stage s={s} at full width and depth "
+                        f"({L} blocks, D={D}, H={H}, T={T}), micro-batch 1 instead of {c['mu']} ({mu * T} tokens): "
+                        f"F + B (G += g) + AdamW time/{k}; {len(timed)} timed step(s); BLAS threads {threads} "
+                        f"of {host} host cores"))
+    return mu * T / t, info
+
+
+def run_reference(args, c, name):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    val, info = oracle_sample(c, args.steps, args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": info["s_per_step"] * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(name, c)},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
+                             "sample": info["sample"]},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------ CUDA leg
+def build_pipeline(pb, c, device):
+    import synth
+    dt = pb.BF16 if c["dtype"] == "bf16" else pb.FP32
+    stages = []
+    for s in range(c["S"]):
+        st = pb.Stage(pb.make_config(s, c["S"], c["L"], c["D"], c["H"], c["T"], c["mu"], c["k"], c["V"], dt),
+                      device=device)
+        st.load_params(synth.stage_params(SEED, s, c["S"], c["L"], c["D"], c["V"], c["T"]))
+        stages.append(st)
+    return stages, pb.Pipeline(stages)
+
+
+def per_stage_times(pb, torch, c, stages, reps=3):
+    """t_F, t_B, t_step of every stage kind through paci_forward / paci_backward / paci_maybe_step
+    (SURVEY.md 8(d) "Procedure"): tokens/s per stage step = M / (t_F + t_B + t_step / k)."""
+    S, mu, T, D, V, k = c["S"], c["mu"], c["T"], c["D"], c["V"], c["k"]
+    act = torch.bfloat16 if c["dtype"] == "bf16" else torch.float32
+    g = torch.Generator(device="cuda").manual_seed(SEED)
+    out = []
+    mb = 1 << 20
+    for s, st in enumerate(stages):
+        emb, head = s == 0, s == S - 1
+        inp = (torch.randint(0, V, (mu, T), device="cuda", dtype=torch.int32, generator=g) if emb
+               else torch.randn(mu, T, D, device="cuda", generator=g).to(act))
+        tgt = torch.randint(0, V, (mu, T), device="cuda", dtype=torch.int32, generator=g) if head else None
+        o = torch.zeros(1, device="cuda") if head else torch.empty(mu, T, D, device="cuda", dtype=act)
+        dout = None if head else (torch.randn(mu, T, D, device="cuda", generator=g) * 1e-3).to(act)
+        din = None if emb else torch.empty(mu, T, D, device="cuda", dtype=act)
+        tf, tb, tu = [], [], []
+        for r in range(reps + 1):
+            for j in range(k):
+                e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+                e[0].record(); st.forward(mb, inp, tgt, o); e[1].record()
+                st.backward(mb, dout, din); e[2].record()
+                stepped = st.maybe_step(c["lr"]); e[3].record()
+                mb += 1
+                torch.cuda.synchronize()
+                if r > 0:
+                    tf.append(e[0].elapsed_time(e[1])); tb.append(e[1].elapsed_time(e[2]))
+                    if stepped:
+                        tu.append(e[2].elapsed_time(e[3]))
+        f, b, u = float(np.median(tf)), float(np.median(tb)), float(np.median(tu))
+        out.append({"stage": s, "t_fwd_ms": round(f, 4), "t_bwd_ms": round(b, 4), "t_step_ms": round(u, 4),
+                    "tokens_per_s": mu * T / ((f + b + u / k) * 1e-3)})
+    return out
+
+
+def run_ours(args, c, name):
+    import torch
+    from paper_2606_07881_b200 import replicas
+    rank, world, local = replicas.init_from_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = f"cuda:{local}"
+    from paper_2606_07881_b200 import binding as pb
+    import synth
+
+    S, mu, T, n_micro, k = c["S"], c["mu"], c["T"], c["n_micro"], c["k"]
+    tokens_per_step = n_micro * mu * T
+    stages, pipe = build_pipeline(pb, c, device)
+    n_batches = args.warmup + 2 * args.steps
+    tok_host = synth.tokens(SEED + rank, n_batches * n_micro, mu, T, c["V"], c["dist"])
+    tok_host = tok_host.reshape(n_batches, n_micro, mu, T + 1)
+    tok_dev = torch.from_numpy(tok_host).to(device)
+    tok_pinned = torch.from_numpy(tok_host).pin_memory()
+    lr = c["lr"]
+
+    for w in range(args.warmup):                                     # untimed warm-up steps
+        pipe.run(tok_dev[w], lr, want_delta=False)
+
+    # ---- timed region 1: inputs resident in HBM
+    clocks = ClockSampler(local)
+    replicas.barrier(); torch.cuda.synchronize()
+    clocks.start()
+    pb.profile_begin(args.sample_stride)
+    dev_ms, launches = 0.0, 0
+    delta_max, losses = 0, []
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        out = pipe.run(tok_dev[args.warmup + i], lr)
+        dev_ms += out["elapsed_ms"]; launches += out["n_launches"]
+        delta_max = max(delta_max, int(out["delta"].max())); losses.append(float(out["loss"].mean()))
+    torch.cuda.synchronize()
+    wall_ms = (time.perf_counter() - t0) * 1e3
+    prof = pb.profile_end()
+    clk = clocks.stop()
+    replicas.barrier()
+    value, max_ms = replicas.whole_job_throughput(dev_ms, S * tokens_per_step * args.steps)
+    ms_per_step = max_ms / args.steps
+
+    # ---- timed region 2: end to end through the C ABI with HOST token buffers (pinned), loss read back
+    replicas.barrier(); torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        out = pipe.run(tok_pinned[args.warmup + args.steps + i], lr, want_delta=False)
+    torch.cuda.synchronize()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    replicas.barrier()
+    e2e_value, _ = replicas.whole_job_throughput(e2e_ms, S * tokens_per_step * args.steps)
+
+    if rank != 0:
+        return 0
+
+    # ---- roofline of the dominant kernel (the tcgen05 GEMM) from the sampled in-library events
+    peaks = measured_peaks()
+    cats = {}
+    for n, e in prof.items():
+        if e["launches"] == 0:
+            continue
+        d = {"launches": e["launches"], "sampled": e["sampled"], "sampled_ms": round(e["sampled_ms"], 3)}
+        if e["sampled_ms"] > 0:
+            if e["flops"] > 0:
+                d["tflops"] = round(e["sampled_flops"] / e["sampled_ms"] * 1e-9, 1)
+                d["frac"] = round(d["tflops"] / peaks["tf_sustained"], 3)
+            else:
+                d["gbs"] = round(e["sampled_bytes"] / e["sampled_ms"] * 1e-6, 1)
+                d["frac"] = round(d["gbs"] / peaks["hbm"], 3)
+            # this category's estimated share of the step: mean sampled duration x launches
+            d["est_ms_per_step"] = round(e["sampled_ms"] / e["sampled"] * e["launches"] / args.steps, 3)
+        cats[n] = d
+    g = [prof[n] for n in ("gemm_fwd", "gemm_dgrad", "gemm_wgrad")]
+    g_ms = sum(e["sampled_ms"] for e in g)
+    g_flops = sum(e["sampled_flops"] for e in g)
+    g_n = sum(e["sampled"] for e in g)
+    achieved = g_flops / g_ms * 1e-9 if g_ms > 0 else 0.0
+    roofline = {"bound": "tensor", "kernel": "gemm_tc_kernel (tcgen05 bf16, all GEMM launches of the step)",
+                "achieved": round(achieved, 1), "peak": peaks["tf_sustained"], "unit": "TFLOP/s",
+                "frac": round(achieved / peaks["tf_sustained"], 4),
+                "peak_source": f"{peaks['source']} sustained bf16 (kernel timed inside a long step)",
+                "traffic": ncu_traffic("gemm_tc_kernel"),
+                "flops_per_launch": g_flops / g_n if g_n else None,
+                "ms_per_launch": g_ms / g_n if g_n else None,
+                "sampled_launches": g_n, "sample_stride": args.sample_stride}
+
+    stage_times = per_stage_times(pb, torch, c, stages) if not args.no_stage_times else None
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": c["dtype"], "data": "synthetic",
+            "config": {"workload": workload_name(name, c), "n_stages": S, "tokens_per_step": tokens_per_step,
+                       "stage_steps_per_step": S * n_micro,
+                       "l2": "inputs larger than L2 (each step streams > 20 GB of weights and stashed activations)",
+                       "parallelism": "replicas only" if world > 1 else "1 GPU, S emulated stages on per-stage streams",
+                       "gemm_backend": "tcgen05" if pb.lib.paci_gemm_backend_is_tcgen05() else "simt"},
+            "pipeline_tokens_per_s": value / S, "wall_ms_per_step": wall_ms / args.steps,
+            "clocks": clk,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": n_micro * mu * (T + 1) * 4,
+                    "d2h_bytes_per_step": n_micro * 4, "ms_per_step": e2e_ms / args.steps},
+            "gpu_launches": launches,
+            "roofline": roofline, "kernels": cats,
+            "max_crossed_updates": delta_max, "mean_loss_per_step": losses}
+    if stage_times is not None:
+        line["per_stage"] = stage_times
+    if world == 1 and not args.no_cpu_baseline:
+        val, info = oracle_sample(c, 1, 0)
+        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
+                                "sample": info["sample"]}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="medium", choices=sorted(CONFIGS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--sample-stride", type=int, default=11, help="time every n-th library op with CUDA events")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-stage-times", action="store_true")
+    args = ap.parse_args()
+    c = CONFIGS[args.config]
+    if args.impl == "reference":
+        return run_reference(args, c, args.config)
+    return run_ours(args, c, args.config)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

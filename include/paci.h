@@ -228,6 +228,21 @@ int paci_op_adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float*
                   int k, int64_t t, float lr, float beta1, float beta2, float eps, float weight_decay,
                   int64_t* version_word, void* stream);
 
+/* ---- sampled kernel timing (bench.py "roofline") ----------------------------- */
+/* Categories, in order: gemm_fwd, gemm_dgrad, gemm_wgrad, attention_fwd, attention_bwd, layernorm_fwd,
+ * layernorm_bwd, gelu_fwd, gelu_bwd, colsum, embedding, softmax_ce, adamw, other.  flops / bytes are
+ * the ALGORITHMIC work of the op, summed over every launch since
+ * paci_profile_begin; every sample_stride-th launch is bracketed by CUDA events on the stream it is
+ * launched on, and sampled_* sum those launches only (sampled_ms = their device time). */
+#define PACI_PROF_NCAT 14
+typedef struct paci_prof_entry {
+  int64_t launches, sampled;
+  double flops, bytes, sampled_flops, sampled_bytes, sampled_ms;
+} paci_prof_entry;
+int paci_profile_begin(int32_t sample_stride);      /* 0 switches the profiler off                */
+int paci_profile_end(paci_prof_entry* out);         /* HOST [PACI_PROF_NCAT]; synchronises the device */
+const char* paci_profile_category_name(int32_t cat);
+
 /* Number of kernels the library has launched in this process (for bench.py's gpu_launches). */
 int64_t paci_launch_count(void);
 /* 1 if the tcgen05 GEMM path is in use for PACI_BF16 GEMMs, 0 if the SIMT fallback was forced by

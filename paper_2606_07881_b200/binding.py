@@ -34,6 +34,13 @@ class RunReport(C.Structure):
                 ("n_slots", C.c_int64), ("n_launches", C.c_int64), ("elapsed_ms", C.c_float)]
 
 
+class ProfEntry(C.Structure):
+    _fields_ = [("launches", C.c_int64), ("sampled", C.c_int64)] + [(n, C.c_double) for n in (
+        "flops", "bytes", "sampled_flops", "sampled_bytes", "sampled_ms")]
+
+
+PROF_NCAT = 14
+
 # name -> (restype, argtypes); every symbol include/paci.h declares
 _vp, _i, _i64, _sz, _f = C.c_void_p, C.c_int, C.c_int64, C.c_size_t, C.c_float
 SIGNATURES = {
@@ -70,6 +77,9 @@ SIGNATURES = {
     "paci_op_embed_bwd": (_i, [_i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_softmax_ce": (_i, [_i, _i, _i, _i, _vp, _vp, _vp, _vp]),
     "paci_op_adamw": (_i, [_sz, _sz, _vp, _vp, _vp, _vp, _vp, _i, _i64, _f, _f, _f, _f, _f, _vp, _vp]),
+    "paci_profile_begin": (_i, [C.c_int32]),
+    "paci_profile_end": (_i, [C.POINTER(ProfEntry)]),
+    "paci_profile_category_name": (C.c_char_p, [C.c_int32]),
     "paci_launch_count": (_i64, []),
     "paci_gemm_backend_is_tcgen05": (_i, []),
 }
@@ -256,3 +266,15 @@ class Pipeline:
               "paci_pipeline_run")
         return dict(loss=loss, delta=delta, version=version, max_q=max_q, n_slots=rep.n_slots,
                     n_launches=rep.n_launches, elapsed_ms=rep.elapsed_ms)
+
+
+def profile_begin(sample_stride: int):
+    check(lib.paci_profile_begin(sample_stride), "paci_profile_begin")
+
+
+def profile_end() -> dict:
+    """category name -> dict(launches, sampled, flops, bytes, sampled_flops, sampled_bytes, sampled_ms)"""
+    arr = (ProfEntry * PROF_NCAT)()
+    check(lib.paci_profile_end(arr), "paci_profile_end")
+    return {lib.paci_profile_category_name(i).decode(): {f: getattr(arr[i], f) for f, _ in ProfEntry._fields_}
+            for i in range(PROF_NCAT)}

@@ -98,6 +98,16 @@ static inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) 
 static inline size_t align_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
 
 int num_sms();
+
+// ---------------------------------------------------------------- sampled kernel timing (prof.cu)
+enum ProfCat { PC_GEMM_FWD = 0, PC_GEMM_DGRAD, PC_GEMM_WGRAD, PC_ATTN_FWD, PC_ATTN_BWD, PC_LN_FWD, PC_LN_BWD,
+               PC_GELU_FWD, PC_GELU_BWD, PC_COLSUM, PC_EMBED, PC_SOFTMAX_CE, PC_ADAMW, PC_OTHER };
+struct ProfScope {   // counts the launch; every stride-th one is timed with events on stream s
+  ProfScope(int cat, double flops, double bytes, cudaStream_t s);
+  ~ProfScope();
+  int idx_;
+  cudaStream_t stream_;
+};
 int stage_cfg_field(const ::paci_stage* st, int field);   // i-th int32 of the stage's paci_stage_config
 
 // ---------------------------------------------------------------- kernel launchers (host)

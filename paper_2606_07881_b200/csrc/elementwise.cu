@@ -130,6 +130,8 @@ static int ln_fwd_t(int rows, int D, const void* x, const void* res, const float
 int ln_fwd(int dtype, int rows, int D, const void* x, const void* res, const float* g, const float* b,
            void* xsum, void* y, float* mean, float* rstd, cudaStream_t s) {
   if (rows <= 0) return PACI_OK;
+  const double e = dtype == PACI_BF16 ? 2.0 : 4.0;
+  ProfScope prof(PC_LN_FWD, 0.0, e * rows * (double)D * (2 + (res != nullptr) + (xsum != nullptr)) + 8.0 * rows, s);
   return dtype == PACI_BF16 ? ln_fwd_t<bf16>(rows, D, x, res, g, b, xsum, y, mean, rstd, s)
                             : ln_fwd_t<float>(rows, D, x, res, g, b, xsum, y, mean, rstd, s);
 }
@@ -256,6 +258,8 @@ static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float*
 int ln_bwd(int dtype, int rows, int D, const void* dy, const void* x, const float* mean, const float* rstd,
            const float* g, const void* dres, void* dx, float* Gg, float* Gb, float* Gcol, cudaStream_t s) {
   if (rows <= 0) return PACI_OK;
+  const double e = dtype == PACI_BF16 ? 2.0 : 4.0;
+  ProfScope prof(PC_LN_BWD, 0.0, e * rows * (double)D * (3 + (dres != nullptr)) + 8.0 * rows, s);
   return dtype == PACI_BF16 ? ln_bwd_t<bf16>(rows, D, dy, x, mean, rstd, g, dres, dx, Gg, Gb, Gcol, s)
                             : ln_bwd_t<float>(rows, D, dy, x, mean, rstd, g, dres, dx, Gg, Gb, Gcol, s);
 }
@@ -285,6 +289,7 @@ __global__ void __launch_bounds__(256) gelu_fwd_kernel(size_t nvec, const T* __r
 
 int gelu_fwd(int dtype, size_t n, const void* p, void* out, cudaStream_t s) {
   if (n == 0) return PACI_OK;
+  ProfScope prof(PC_GELU_FWD, 0.0, (dtype == PACI_BF16 ? 2.0 : 4.0) * 2.0 * (double)n, s);
   const int V = dtype == PACI_BF16 ? 8 : 4;
   if (n % V) return fail(PACI_EINVAL, "gelu: n not a multiple of %d", V);
   const size_t nvec = n / V;
@@ -351,9 +356,11 @@ static int colslab(int dtype, int rows, int cols, const void* a, const void* p, 
 
 int gelu_bwd(int dtype, int rows, int cols, const void* dg, const void* p, void* dp, float* Gbias,
              cudaStream_t s) {
+  ProfScope prof(PC_GELU_BWD, 0.0, (dtype == PACI_BF16 ? 2.0 : 4.0) * 3.0 * rows * (double)cols, s);
   return colslab<true>(dtype, rows, cols, dg, p, dp, Gbias, s);
 }
 int colsum(int dtype, int rows, int cols, const void* x, float* G, cudaStream_t s) {
+  ProfScope prof(PC_COLSUM, 0.0, (dtype == PACI_BF16 ? 2.0 : 4.0) * rows * (double)cols, s);
   return colslab<false>(dtype, rows, cols, x, nullptr, nullptr, G, s);
 }
 
@@ -379,6 +386,7 @@ __global__ void __launch_bounds__(256) embed_fwd_kernel(int M, int T_, int D, co
 
 int embed_fwd(int dtype, int mu, int T_, int D, const int32_t* tok, const float* wte, const float* wpe, void* x,
               cudaStream_t s) {
+  ProfScope prof(PC_EMBED, 0.0, ((dtype == PACI_BF16 ? 2.0 : 4.0) + 4.0) * mu * (double)T_ * D + 4.0 * T_ * D, s);
   const int M = mu * T_;
   const int V = dtype == PACI_BF16 ? 8 : 4;
   if (D % V) return fail(PACI_EINVAL, "embed: D=%d", D);
@@ -433,6 +441,8 @@ __global__ void __launch_bounds__(256) embed_bwd_wpe_kernel(int mu, int T_, int 
 
 int embed_bwd(int dtype, int mu, int T_, int D, const int32_t* tok, const void* dx, float* Gwte, float* Gwpe,
               cudaStream_t s) {
+  // dx read twice (wte scatter, wpe reduction) + fp32 read-modify-write of the touched rows
+  ProfScope prof(PC_EMBED, 0.0, ((dtype == PACI_BF16 ? 2.0 : 4.0) * 2.0 + 8.0) * mu * (double)T_ * D + 8.0 * T_ * D, s);
   const int M = mu * T_;
   const int V = dtype == PACI_BF16 ? 8 : 4;
   if (D % V) return fail(PACI_EINVAL, "embed_bwd: D=%d", D);
@@ -520,6 +530,7 @@ __global__ void __launch_bounds__(512) softmax_ce_kernel(int rows, int V_, int l
 }
 
 int softmax_ce(int dtype, int rows, int V_, int ldz, void* z, const int32_t* tgt, float* loss, cudaStream_t s) {
+  ProfScope prof(PC_SOFTMAX_CE, 0.0, (dtype == PACI_BF16 ? 2.0 : 4.0) * 2.0 * rows * (double)ldz, s);
   const int V = dtype == PACI_BF16 ? 8 : 4;
   if (ldz % V || ldz < V_) return fail(PACI_EINVAL, "softmax_ce: ldz=%d V=%d", ldz, V_);
   if (dtype == PACI_BF16) PACI_LAUNCH(softmax_ce_kernel<bf16>, rows, 512, 0, s, rows, V_, ldz, (bf16*)z, tgt, loss);
@@ -568,6 +579,7 @@ __global__ void __launch_bounds__(256) adamw_kernel(size_t n4, size_t n4_decay, 
 
 int adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float* G, void* shadow, int k, int64_t t,
           float lr, float beta1, float beta2, float eps, float wd, int64_t* version_word, cudaStream_t s) {
+  ProfScope prof(PC_ADAMW, 0.0, (shadow != nullptr ? 34.0 : 32.0) * (double)n, s);
   if (n % 4 || n_decay % 4) return fail(PACI_EINVAL, "adamw: n=%zu n_decay=%zu must be multiples of 4", n, n_decay);
   const double bc1 = 1.0 - std::pow((double)beta1, (double)t), bc2 = 1.0 - std::pow((double)beta2, (double)t);
   const size_t n4 = n / 4;
@@ -584,6 +596,7 @@ __global__ void cast_shadow_kernel(size_t n, const float* __restrict__ w, bf16* 
 }
 int cast_shadow(size_t n, const float* w, void* shadow, cudaStream_t s) {
   if (n == 0) return PACI_OK;
+  ProfScope prof(PC_OTHER, 0.0, 6.0 * (double)n, s);
   int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)num_sms() * 8);
   PACI_LAUNCH(cast_shadow_kernel, blocks, 256, 0, s, n, w, (bf16*)shadow);
   return PACI_OK;
@@ -607,6 +620,7 @@ __global__ void __launch_bounds__(256) add_vec_kernel(size_t nvec, const T* __re
 }
 int add_vec(int dtype, size_t n, const void* a, const void* b, void* out, cudaStream_t s) {
   if (n == 0) return PACI_OK;
+  ProfScope prof(PC_OTHER, 0.0, (dtype == PACI_BF16 ? 2.0 : 4.0) * (double)n * (2 + (b != nullptr)), s);
   const int V = dtype == PACI_BF16 ? 8 : 4;
   if (n % V) return fail(PACI_EINVAL, "add: n not a multiple of %d", V);
   const size_t nvec = n / V;

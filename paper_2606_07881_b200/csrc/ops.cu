@@ -25,6 +25,9 @@ static bool attn_backend_tensor() {
 
 int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
          const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s) {
+  const double e = dtype == PACI_BF16 ? 2.0 : 4.0;
+  ProfScope prof(layout == 0 ? PC_GEMM_FWD : layout == 1 ? PC_GEMM_DGRAD : PC_GEMM_WGRAD, 2.0 * M * N * K,
+                 e * ((double)M * K + (double)N * K) + (out_f32_accum ? 8.0 : e) * M * N, s);
   if (dtype == PACI_BF16 && gemm_backend_tcgen05())
     return gemm_tc(layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, s);
   return gemm_simt(dtype, layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, s);
@@ -35,7 +38,10 @@ int attention_bwd_mma(int mu, int T, int H, const void* dout, const void* qkv, c
                       void* dqkv, float* scratch, cudaStream_t s);
 size_t attention_bwd_mma_scratch_bytes(int mu, int T, int H);
 
+// algorithmic work: causal half of QK^T and PV (2 * mu*H*T*T*dh flops forward, twice that backward)
 int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse, cudaStream_t s) {
+  const double e = dtype == PACI_BF16 ? 2.0 : 4.0, nd = (double)mu * T * H * dh;
+  ProfScope prof(PC_ATTN_FWD, 2.0 * mu * H * (double)T * T * dh, e * 4.0 * nd + 4.0 * mu * H * T, s);
   if (dtype == PACI_BF16 && attn_backend_tensor()) {
     if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
     return attention_fwd_mma(mu, T, H, qkv, o, lse, s);
@@ -45,6 +51,8 @@ int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void
 
 int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv, const void* o,
                   const float* lse, void* dqkv, float* scratch, cudaStream_t s) {
+  const double e = dtype == PACI_BF16 ? 2.0 : 4.0, nd = (double)mu * T * H * dh;
+  ProfScope prof(PC_ATTN_BWD, 4.0 * mu * H * (double)T * T * dh, e * 8.0 * nd + 4.0 * mu * H * T, s);
   if (dtype == PACI_BF16 && attn_backend_tensor()) {
     if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
     return attention_bwd_mma(mu, T, H, dout, qkv, o, lse, dqkv, scratch, s);
