@@ -22,6 +22,7 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <cstdlib>
 #include <mutex>
 #include <unordered_map>
 
@@ -34,8 +35,8 @@ namespace {
 constexpr int BLOCK_M = 128;
 constexpr int BLOCK_K = 64;
 constexpr int UMMA_K = 16;
-constexpr int STAGES = 4;
 constexpr int NUM_THREADS = 192;
+constexpr uint32_t EPI_STAGING_BYTES = 4 * 2 * 4096;
 
 // ------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -86,6 +87,70 @@ __device__ __forceinline__ void umma_commit(uint64_t* bar) {   // arrives on bar
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
                : "memory");
 }
+// ---- CTA-pair (cta_group::2) variants: two SMs of one TPC execute one M=256 MMA; each CTA stages its own
+// 128 rows of A and HALF of the B tile, so the shared-memory fill per FLOP is 2/3 of the 1-CTA kernel's.
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t mapa_rank(uint32_t saddr, uint32_t rank) {   // same offset in CTA `rank`
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// TMA load issued by either CTA of the pair; the bytes are counted on the LEADER's mbarrier (cluster address)
+__device__ __forceinline__ void tma_load_2d_pair(void* dst, const CUtensorMap* map, uint32_t leader_bar, int c0,
+                                                 int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(smem_u32(dst)), "l"(map), "r"(leader_bar), "r"(c0), "r"(c1)
+      : "memory");
+}
+__device__ __forceinline__ void umma_bf16_pair(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc,
+                                               uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+      : "memory");
+}
+__device__ __forceinline__ void umma_commit_pair(uint64_t* bar) {   // arrives on `bar` in BOTH CTAs of the pair
+  asm volatile(
+      "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+      ::"r"(smem_u32(bar)), "h"((uint16_t)3)
+      : "memory");
+}
+// ---- epilogue: registers -> 128B-swizzled shared memory -> TMA store (bf16) or TMA reduce-add (fp32, beta = 1)
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, const void* src, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+               ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_reduce_add_2d(const CUtensorMap* map, const void* src, int c0, int c1) {
+  asm volatile("cp.reduce.async.bulk.tensor.2d.global.shared::cta.add.bulk_group [%0, {%2, %3}], [%1];"
+               ::"l"(map), "r"(smem_u32(src)), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void bulk_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void sts128(void* dst, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(smem_u32(dst)), "r"(a), "r"(b), "r"(c), "r"(d)
+               : "memory");
+}
+__device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
+  __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&v);
+}
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
   asm volatile(
       "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
@@ -118,85 +183,121 @@ struct Params {
 };
 
 // ------------------------------------------------------------------ the kernel
-template <int BLOCK_N, bool A_MN, bool B_MN, bool ACCUM>
+// CG = 1: one CTA per tile of 128 x BLOCK_N.  CG = 2: a CTA pair (cluster of 2, same TPC) per tile of
+// 256 x BLOCK_N: CTA r owns rows m0 + 128 r .. of A and of the accumulator, and stages columns
+// n0 + r BLOCK_N/2 .. of B; the leader (rank 0) issues tcgen05.mma.cta_group::2 for both.
+template <int CG, int BLOCK_N, int STAGES, bool A_MN, bool B_MN, bool ACCUM>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
-gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const Params p) {
-  constexpr uint32_t A_BYTES = BLOCK_M * BLOCK_K * 2, B_BYTES = BLOCK_N * BLOCK_K * 2;
+gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
+               const __grid_constant__ CUtensorMap tmC, const Params p) {
+  constexpr int BN_CTA = BLOCK_N / CG;                  // B rows staged by one CTA
+  constexpr uint32_t A_BYTES = BLOCK_M * BLOCK_K * 2, B_BYTES = BN_CTA * BLOCK_K * 2;
   constexpr uint32_t STAGE_BYTES = A_BYTES + B_BYTES;
   constexpr uint32_t BOX_MN_BYTES = 64 * BLOCK_K * 2;   // one {64 mn, 64 k} box of an MN-major operand
   constexpr uint32_t TMEM_COLS = 2 * BLOCK_N;
   // instruction descriptor: D fp32 (bit 4), A/B bf16 (bits 7, 10), majors (15, 16), N>>3 at 17, M>>4 at 24
   constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((A_MN ? 1u : 0u) << 15) |
                              ((B_MN ? 1u : 0u) << 16) | ((uint32_t)(BLOCK_N >> 3) << 17) |
-                             ((uint32_t)(BLOCK_M >> 4) << 24);
+                             ((uint32_t)((BLOCK_M * CG) >> 4) << 24);
 
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint64_t* full = (uint64_t*)(smem + STAGES * STAGE_BYTES);
+  uint8_t* staging = smem + STAGES * STAGE_BYTES;        // 4 epilogue warps x 2 buffers x 4 KB (1024-aligned)
+  float* bias_s = (float*)(staging + EPI_STAGING_BYTES); // 4 epilogue warps x BLOCK_N floats
+  uint64_t* full = (uint64_t*)(bias_s + 4 * BLOCK_N);
   uint64_t* empty = full + STAGES;
   uint64_t* tfull = empty + STAGES;
   uint64_t* tempty = tfull + 2;
   uint32_t* tmem_slot = (uint32_t*)(tempty + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = CG == 2 ? cluster_ctarank() : 0u;
+  const bool leader = rank == 0;
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < STAGES; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 4); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 4 * CG); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
-                 "r"(TMEM_COLS)
-                 : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (CG == 2) {
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
+                   "r"(TMEM_COLS) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
+                   "r"(TMEM_COLS) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
   }
   tc_fence_before();
   __syncthreads();
+  if (CG == 2) cluster_sync_all();                       // the peer's barriers exist before anything signals them
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
   const int n_items = p.tiles_m * p.tiles_n * p.splits;
   const int kb_per = (p.kb_total + p.splits - 1) / p.splits;
+  const int worker = CG == 2 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
+  const int n_workers = CG == 2 ? (int)(gridDim.x >> 1) : (int)gridDim.x;
 
   if (warp == 0) {
     if (lane == 0) {
       asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
       asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
       uint32_t stage = 0, phase = 0;
-      for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+      for (int item = worker; item < n_items; item += n_workers) {
         const int tile = item / p.splits, split = item % p.splits;
-        const int m0 = (tile % p.tiles_m) * BLOCK_M, n0 = (tile / p.tiles_m) * BLOCK_N;
+        const int m0 = (tile % p.tiles_m) * (BLOCK_M * CG) + (int)rank * BLOCK_M;
+        const int n0 = (tile / p.tiles_m) * BLOCK_N + (int)rank * BN_CTA;
         const int kb0 = split * kb_per, kb1 = min(kb0 + kb_per, p.kb_total);
         for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(&empty[stage], phase ^ 1);
           uint8_t* sa = smem + stage * STAGE_BYTES;
           uint8_t* sb = sa + A_BYTES;
-          mbar_expect_tx(&full[stage], STAGE_BYTES);
           const int k0 = kb * BLOCK_K;
-          if (A_MN) {
+          if (CG == 2) {
+            // both CTAs' bytes are counted on the leader's barrier; its single arrival is this expect_tx
+            if (leader) mbar_expect_tx(&full[stage], 2 * STAGE_BYTES);
+            const uint32_t bar = mapa_rank(smem_u32(&full[stage]), 0);
+            if (A_MN) {
 #pragma unroll
-            for (int i = 0; i < BLOCK_M / 64; ++i) tma_load_2d(sa + i * BOX_MN_BYTES, &tmA, &full[stage], m0 + i * 64, k0);
-          } else {
-            tma_load_2d(sa, &tmA, &full[stage], k0, m0);
-          }
-          if (B_MN) {
+              for (int i = 0; i < BLOCK_M / 64; ++i) tma_load_2d_pair(sa + i * BOX_MN_BYTES, &tmA, bar, m0 + i * 64, k0);
+            } else {
+              tma_load_2d_pair(sa, &tmA, bar, k0, m0);
+            }
+            if (B_MN) {
 #pragma unroll
-            for (int i = 0; i < BLOCK_N / 64; ++i) tma_load_2d(sb + i * BOX_MN_BYTES, &tmB, &full[stage], n0 + i * 64, k0);
+              for (int i = 0; i < BN_CTA / 64; ++i) tma_load_2d_pair(sb + i * BOX_MN_BYTES, &tmB, bar, n0 + i * 64, k0);
+            } else {
+              tma_load_2d_pair(sb, &tmB, bar, k0, n0);
+            }
           } else {
-            tma_load_2d(sb, &tmB, &full[stage], k0, n0);
+            mbar_expect_tx(&full[stage], STAGE_BYTES);
+            if (A_MN) {
+#pragma unroll
+              for (int i = 0; i < BLOCK_M / 64; ++i) tma_load_2d(sa + i * BOX_MN_BYTES, &tmA, &full[stage], m0 + i * 64, k0);
+            } else {
+              tma_load_2d(sa, &tmA, &full[stage], k0, m0);
+            }
+            if (B_MN) {
+#pragma unroll
+              for (int i = 0; i < BN_CTA / 64; ++i) tma_load_2d(sb + i * BOX_MN_BYTES, &tmB, &full[stage], n0 + i * 64, k0);
+            } else {
+              tma_load_2d(sb, &tmB, &full[stage], k0, n0);
+            }
           }
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    if (lane == 0) {
+    if (lane == 0 && leader) {
       uint32_t stage = 0, phase = 0, acc = 0, acc_phase = 0;
-      for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+      for (int item = worker; item < n_items; item += n_workers) {
         const int split = item % p.splits;
         const int kb0 = split * kb_per, kb1 = min(kb0 + kb_per, p.kb_total);
-        mbar_wait(&tempty[acc], acc_phase ^ 1);      // epilogue has drained this accumulator
+        mbar_wait(&tempty[acc], acc_phase ^ 1);      // epilogue (of both CTAs) has drained this accumulator
         tc_fence_after();
         const uint32_t tmem_d = tmem_base + acc * BLOCK_N;
         for (int kb = kb0; kb < kb1; ++kb) {
@@ -209,83 +310,101 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
                                      : smem_desc(sa + j * (UMMA_K * 2), 16, 1024);
             const uint64_t bd = B_MN ? smem_desc(sb + j * (UMMA_K * 128), BOX_MN_BYTES, 1024)
                                      : smem_desc(sb + j * (UMMA_K * 2), 16, 1024);
-            umma_bf16(tmem_d, ad, bd, IDESC, (kb > kb0 || j > 0) ? 1u : 0u);
+            if (CG == 2) umma_bf16_pair(tmem_d, ad, bd, IDESC, (kb > kb0 || j > 0) ? 1u : 0u);
+            else umma_bf16(tmem_d, ad, bd, IDESC, (kb > kb0 || j > 0) ? 1u : 0u);
           }
-          umma_commit(&empty[stage]);                 // frees the smem stage when these MMAs retire
+          if (CG == 2) umma_commit_pair(&empty[stage]); else umma_commit(&empty[stage]);   // frees the stage
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
-        umma_commit(&tfull[acc]);                     // accumulator complete -> epilogue
+        if (CG == 2) umma_commit_pair(&tfull[acc]); else umma_commit(&tfull[acc]);         // -> epilogue
         acc ^= 1;
         if (acc == 0) acc_phase ^= 1;
       }
     }
   } else {
-    const int q = warp & 3;                           // TMEM lane quarter this warp may access
-    uint32_t acc = 0, acc_phase = 0;
-    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+    // ===== epilogue warps: TMEM -> registers -> swizzled smem -> TMA store / TMA reduce-add =====
+    // Warp w (TMEM lane quarter q = w & 3) owns 32 rows of the tile and a private pair of 4 KB staging
+    // buffers, so the four warps never synchronise with each other.  One TMA box = 32 rows x 128 bytes
+    // (64 bf16 or 32 fp32 columns), SWIZZLE_128B: 16-byte chunk c of row r sits at chunk c ^ (r & 7),
+    // which makes the row-per-thread st.shared.v4 conflict-free.  TMA clips the box at the tensor edge.
+    const int q = warp & 3;
+    constexpr int CHUNK = ACCUM ? 32 : 64;            // columns per TMA box
+    uint8_t* my_stage = staging + (warp - 2) * 8192;
+    float* my_bias = bias_s + (warp - 2) * BLOCK_N;
+    uint32_t acc = 0, acc_phase = 0, sbuf = 0;
+    for (int item = worker; item < n_items; item += n_workers) {
       const int tile = item / p.splits;
-      const int m0 = (tile % p.tiles_m) * BLOCK_M, n0 = (tile / p.tiles_m) * BLOCK_N;
+      const int m0 = (tile % p.tiles_m) * (BLOCK_M * CG) + (int)rank * BLOCK_M, n0 = (tile / p.tiles_m) * BLOCK_N;
+      if (!ACCUM) {                                   // bias slice of this tile, fetched under the main loop
+#pragma unroll
+        for (int i = 0; i < BLOCK_N / 32; ++i) {
+          const int col = n0 + i * 32 + lane;
+          my_bias[i * 32 + lane] = (p.bias != nullptr && col < p.N) ? __ldg(p.bias + col) : 0.f;
+        }
+        __syncwarp();
+      }
       mbar_wait(&tfull[acc], acc_phase);
       tc_fence_after();
-      const int row = m0 + q * 32 + lane;
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BLOCK_N;
 #pragma unroll 1
-      for (int c = 0; c < BLOCK_N; c += 32) {
+      for (int c = 0; c < BLOCK_N; c += CHUNK) {
         if (n0 + c >= p.N) break;                     // warp-uniform
-        uint32_t r[32];
-        tmem_ld32(taddr + c, r);
-        if (row < p.M) {
-          const int col = n0 + c;
-          if (ACCUM) {
-            float* dst = reinterpret_cast<float*>(p.C) + (size_t)row * p.ldc + col;
+        uint8_t* buf = my_stage + sbuf * 4096;
+        sbuf ^= 1;
+        if (lane == 0) bulk_wait_read<1>();           // the box stored from this buffer two chunks ago is read
+        __syncwarp();
+        uint8_t* rowp = buf + lane * 128;
+        if (ACCUM) {
+          uint32_t r[32];
+          tmem_ld32(taddr + c, r);
 #pragma unroll
-            for (int j = 0; j < 32; j += 4) {
-              if (col + j + 4 <= p.N) {
-                asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + j),
-                             "f"(__uint_as_float(r[j])), "f"(__uint_as_float(r[j + 1])),
-                             "f"(__uint_as_float(r[j + 2])), "f"(__uint_as_float(r[j + 3]))
-                             : "memory");
-              } else {
-                for (int t = 0; t < 4; ++t)
-                  if (col + j + t < p.N) atomicAdd(dst + j + t, __uint_as_float(r[j + t]));
-              }
-            }
-          } else {
-            bf16* dst = reinterpret_cast<bf16*>(p.C) + (size_t)row * p.ldc + col;
+          for (int i = 0; i < 8; ++i)
+            sts128(rowp + ((i ^ (lane & 7)) << 4), r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
+        } else {
 #pragma unroll
-            for (int j = 0; j < 32; j += 8) {
-              float v[8];
+          for (int h = 0; h < 2; ++h) {
+            uint32_t r[32];
+            tmem_ld32(taddr + c + 32 * h, r);
 #pragma unroll
-              for (int t = 0; t < 8; ++t) v[t] = __uint_as_float(r[j + t]);
-              if (col + j + 8 <= p.N) {
-                if (p.bias != nullptr) {
-                  const float4 b0 = __ldg(reinterpret_cast<const float4*>(p.bias + col + j));
-                  const float4 b1 = __ldg(reinterpret_cast<const float4*>(p.bias + col + j + 4));
-                  v[0] += b0.x; v[1] += b0.y; v[2] += b0.z; v[3] += b0.w;
-                  v[4] += b1.x; v[5] += b1.y; v[6] += b1.z; v[7] += b1.w;
-                }
-                store_vec<bf16>(dst + j, v);
-              } else {
-                for (int t = 0; t < 8; ++t)
-                  if (col + j + t < p.N)
-                    dst[j + t] = __float2bfloat16_rn(v[t] + (p.bias != nullptr ? p.bias[col + j + t] : 0.f));
-              }
+            for (int i = 0; i < 4; ++i) {
+              const float4 b0 = *reinterpret_cast<const float4*>(my_bias + c + 32 * h + 8 * i);
+              const float4 b1 = *reinterpret_cast<const float4*>(my_bias + c + 32 * h + 8 * i + 4);
+              const uint32_t w0 = pack_bf16x2(__uint_as_float(r[8 * i]) + b0.x, __uint_as_float(r[8 * i + 1]) + b0.y);
+              const uint32_t w1 = pack_bf16x2(__uint_as_float(r[8 * i + 2]) + b0.z, __uint_as_float(r[8 * i + 3]) + b0.w);
+              const uint32_t w2 = pack_bf16x2(__uint_as_float(r[8 * i + 4]) + b1.x, __uint_as_float(r[8 * i + 5]) + b1.y);
+              const uint32_t w3 = pack_bf16x2(__uint_as_float(r[8 * i + 6]) + b1.z, __uint_as_float(r[8 * i + 7]) + b1.w);
+              sts128(rowp + (((4 * h + i) ^ (lane & 7)) << 4), w0, w1, w2, w3);
             }
           }
+        }
+        fence_async_smem();                           // generic-proxy writes -> visible to the TMA engine
+        __syncwarp();
+        if (lane == 0) {
+          if (ACCUM) tma_reduce_add_2d(&tmC, buf, n0 + c, m0 + q * 32);
+          else tma_store_2d(&tmC, buf, n0 + c, m0 + q * 32);
+          bulk_commit();
         }
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&tempty[acc]);
+      if (lane == 0) {
+        if (CG == 2) mbar_arrive_cluster(mapa_rank(smem_u32(&tempty[acc]), 0));
+        else mbar_arrive(&tempty[acc]);
+      }
       acc ^= 1;
       if (acc == 0) acc_phase ^= 1;
     }
+    if (lane == 0) bulk_wait_all();                   // smem must outlive the last TMA read
   }
   tc_fence_before();
   __syncthreads();
+  if (CG == 2) cluster_sync_all();                     // no CTA leaves while its pair can still signal it
   if (warp == 1) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    if (CG == 2)
+      asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    else
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
   }
 }
 
@@ -308,24 +427,26 @@ EncodeTiledFn encode_fn() {
 }
 
 struct MapKey {
-  const void* ptr; uint64_t d0, d1, ld; uint32_t b0, b1;
+  const void* ptr; uint64_t d0, d1, ld; uint32_t b0, b1, esz;
   bool operator==(const MapKey& o) const {
-    return ptr == o.ptr && d0 == o.d0 && d1 == o.d1 && ld == o.ld && b0 == o.b0 && b1 == o.b1;
+    return ptr == o.ptr && d0 == o.d0 && d1 == o.d1 && ld == o.ld && b0 == o.b0 && b1 == o.b1 && esz == o.esz;
   }
 };
 struct MapKeyHash {
   size_t operator()(const MapKey& k) const {
     size_t h = (size_t)k.ptr;
-    for (uint64_t v : {k.d0, k.d1, k.ld, (uint64_t)k.b0, (uint64_t)k.b1}) h = h * 1000003u ^ (size_t)v;
+    for (uint64_t v : {k.d0, k.d1, k.ld, (uint64_t)k.b0, (uint64_t)k.b1, (uint64_t)k.esz}) h = h * 1000003u ^ (size_t)v;
     return h;
   }
 };
 
-// 2D bf16 tensor: dim0 (contiguous) extent d0, dim1 extent d1 with row stride ld elements; box {b0, b1}.
-int make_map(CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64_t ld, uint32_t b0, uint32_t b1) {
+// 2D tensor of bf16 (esz 2) or fp32 (esz 4): dim0 (contiguous) extent d0, dim1 extent d1 with row stride ld
+// elements; box {b0, b1}; 128-byte swizzle.
+int make_map(CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64_t ld, uint32_t b0, uint32_t b1,
+             uint32_t esz = 2) {
   static std::unordered_map<MapKey, CUtensorMap, MapKeyHash> cache;
   static std::mutex mu;
-  MapKey key{ptr, d0, d1, ld, b0, b1};
+  MapKey key{ptr, d0, d1, ld, b0, b1, esz};
   {
     std::lock_guard<std::mutex> g(mu);
     auto it = cache.find(key);
@@ -333,12 +454,12 @@ int make_map(CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64
   }
   EncodeTiledFn fn = encode_fn();
   if (!fn) return fail(PACI_ECUDA, "cuTensorMapEncodeTiled is not available from the driver");
-  if ((uintptr_t)ptr % 16 || (ld * 2) % 16) return fail(PACI_EINVAL, "tcgen05 GEMM: operand not 16-byte aligned (ld=%llu)", (unsigned long long)ld);
+  if ((uintptr_t)ptr % 16 || (ld * esz) % 16) return fail(PACI_EINVAL, "tcgen05 GEMM: operand not 16-byte aligned (ld=%llu)", (unsigned long long)ld);
   cuuint64_t dims[2] = {d0, d1};
-  cuuint64_t strides[1] = {ld * 2};
+  cuuint64_t strides[1] = {ld * esz};
   cuuint32_t box[2] = {b0, b1};
   cuuint32_t estr[2] = {1, 1};
-  CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
+  CUresult r = fn(out, esz == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr), dims, strides, box, estr,
                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return fail(PACI_ECUDA, "cuTensorMapEncodeTiled failed with %d", (int)r);
@@ -348,17 +469,43 @@ int make_map(CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64
   return PACI_OK;
 }
 
-template <int BLOCK_N, bool A_MN, bool B_MN, bool ACCUM>
-int launch(const CUtensorMap& tmA, const CUtensorMap& tmB, const Params& p, int grid, cudaStream_t s) {
-  constexpr size_t SMEM = (size_t)STAGES * (BLOCK_M * BLOCK_K * 2 + BLOCK_N * BLOCK_K * 2) + 1024 + 256;
-  auto kern = gemm_tc_kernel<BLOCK_N, A_MN, B_MN, ACCUM>;
+
+template <int CG, int BLOCK_N, int STAGES, bool A_MN, bool B_MN, bool ACCUM>
+int launch(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmC, const Params& p, int grid,
+           cudaStream_t s) {
+  constexpr size_t SMEM = (size_t)STAGES * (BLOCK_M * BLOCK_K * 2 + (BLOCK_N / CG) * BLOCK_K * 2) +
+                          EPI_STAGING_BYTES + 4 * BLOCK_N * 4 + 1024 + 256;
+  static_assert(SMEM <= 232448, "shared memory budget of one sm_100 CTA");
+  auto kern = gemm_tc_kernel<CG, BLOCK_N, STAGES, A_MN, B_MN, ACCUM>;
   static bool attr_set = false;
   if (!attr_set) {
     PACI_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
     attr_set = true;
   }
-  PACI_LAUNCH(kern, grid, NUM_THREADS, SMEM, s, tmA, tmB, p);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid);
+  cfg.blockDim = dim3(NUM_THREADS);
+  cfg.dynamicSmemBytes = SMEM;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = CG;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  PACI_CUDA_OK(cudaLaunchKernelEx(&cfg, kern, tmA, tmB, tmC, p));
+  g_launches.fetch_add(1, std::memory_order_relaxed);
   return PACI_OK;
+}
+
+// PACI_GEMM_CG=1 selects the single-CTA kernel (A/B comparison aid); default is the CTA-pair kernel.
+int cta_group() {
+  static const int cg = [] {
+    const char* e = std::getenv("PACI_GEMM_CG");
+    return (e != nullptr && e[0] == '1') ? 1 : 2;
+  }();
+  return cg;
 }
 
 }  // namespace
@@ -372,35 +519,59 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
     return fail(PACI_EINVAL, "tcgen05 GEMM: C not 16-byte aligned (ldc=%d)", ldc);
   if (bias != nullptr && (uintptr_t)bias % 16) return fail(PACI_EINVAL, "tcgen05 GEMM: bias not 16-byte aligned");
   const bool a_mn = layout == 2, b_mn = layout != 0;
+  const int CG = cta_group();
   const int BN = N <= 128 ? 128 : 256;
-  CUtensorMap tmA, tmB;
+  CUtensorMap tmA, tmB, tmC;
   int rc;
   // A: K-major [M rows][K contiguous] -> dims {K, M}, box {64, 128};  MN-major [K rows][M contiguous] -> {M, K}, {64, 64}
   rc = a_mn ? make_map(&tmA, A, M, K, lda, 64, BLOCK_K) : make_map(&tmA, A, K, M, lda, BLOCK_K, BLOCK_M);
   if (rc) return rc;
-  rc = b_mn ? make_map(&tmB, B, N, K, ldb, 64, BLOCK_K) : make_map(&tmB, B, K, N, ldb, BLOCK_K, BN);
+  rc = b_mn ? make_map(&tmB, B, N, K, ldb, 64, BLOCK_K) : make_map(&tmB, B, K, N, ldb, BLOCK_K, BN / CG);
+  if (rc) return rc;
+  // C: box of 32 rows x 128 bytes, written by one epilogue warp per TMA store / reduce-add
+  rc = out_f32_accum ? make_map(&tmC, C, N, M, ldc, 32, 32, 4) : make_map(&tmC, C, N, M, ldc, 64, 32, 2);
   if (rc) return rc;
   Params p;
   p.M = M; p.N = N; p.K = K; p.ldc = ldc; p.bias = bias; p.C = C;
-  p.tiles_m = ceil_div(M, BLOCK_M);
+  p.tiles_m = ceil_div(M, BLOCK_M * CG);
   p.tiles_n = ceil_div(N, BN);
   p.kb_total = ceil_div(K, BLOCK_K);
-  const int tiles = p.tiles_m * p.tiles_n, sms = num_sms();
+  const int tiles = p.tiles_m * p.tiles_n, workers = std::max(1, num_sms() / CG);
   int splits = 1;
-  if (out_f32_accum) {   // split-K over the contraction (tokens): partials meet in the fp32 red.add epilogue
-    splits = std::max(1, std::min({ceil_div(2 * sms, tiles), p.kb_total / 4, 32}));
-    const int kb_per = ceil_div(p.kb_total, splits);
-    splits = ceil_div(p.kb_total, kb_per);            // every split owns at least one k-block
+  if (out_f32_accum) {
+    // split-K over the contraction (tokens): partials meet in the fp32 red.add epilogue.  Pick the split
+    // count that fills whole rounds of the persistent grid best (fewest splits on a tie).
+    const int max_s = std::max(1, std::min(p.kb_total / 4, 32));
+    double best = -1.0;
+    for (int sp = 1; sp <= max_s; ++sp) {
+      const int kb_per = ceil_div(p.kb_total, sp);
+      if (ceil_div(p.kb_total, kb_per) != sp) continue;        // every split owns at least one k-block
+      const long items = (long)tiles * sp;
+      const double eff = (double)items / ((double)ceil_div(items, workers) * workers);
+      if (eff > best + 0.02) { best = eff; splits = sp; }
+    }
   }
   p.splits = splits;
-  const int grid = std::min(tiles * splits, sms);
-#define GO(BN_, AMN, BMN, ACC) return launch<BN_, AMN, BMN, ACC>(tmA, tmB, p, grid, s)
-  if (BN == 128) {
-    if (out_f32_accum) { if (layout == 0) GO(128, false, false, true); if (layout == 1) GO(128, false, true, true); GO(128, true, true, true); }
-    if (layout == 0) GO(128, false, false, false); if (layout == 1) GO(128, false, true, false); GO(128, true, true, false);
+  const int grid = std::min(tiles * splits, workers) * CG;
+#define GO(CG_, BN_, ST_, AMN, BMN, ACC) return launch<CG_, BN_, ST_, AMN, BMN, ACC>(tmA, tmB, tmC, p, grid, s)
+#define BY_LAYOUT(CG_, BN_, ST_)                                                                          \
+  do {                                                                                                    \
+    if (out_f32_accum) {                                                                                  \
+      if (layout == 0) GO(CG_, BN_, ST_, false, false, true);                                             \
+      if (layout == 1) GO(CG_, BN_, ST_, false, true, true);                                              \
+      GO(CG_, BN_, ST_, true, true, true);                                                                \
+    }                                                                                                     \
+    if (layout == 0) GO(CG_, BN_, ST_, false, false, false);                                              \
+    if (layout == 1) GO(CG_, BN_, ST_, false, true, false);                                               \
+    GO(CG_, BN_, ST_, true, true, false);                                                                 \
+  } while (0)
+  if (CG == 2) {
+    if (BN == 128) BY_LAYOUT(2, 128, 7);
+    BY_LAYOUT(2, 256, 5);
   }
-  if (out_f32_accum) { if (layout == 0) GO(256, false, false, true); if (layout == 1) GO(256, false, true, true); GO(256, true, true, true); }
-  if (layout == 0) GO(256, false, false, false); if (layout == 1) GO(256, false, true, false); GO(256, true, true, false);
+  if (BN == 128) BY_LAYOUT(1, 128, 5);
+  BY_LAYOUT(1, 256, 3);
+#undef BY_LAYOUT
 #undef GO
 }
 
