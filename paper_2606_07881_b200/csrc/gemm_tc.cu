@@ -50,10 +50,17 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ uint64_t globaltimer_ns() {
+  uint64_t t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+// A protocol bug must fault, not hang the GPU: a wait that lasts longer than 4 s of wall time traps.
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int tag = 0) {
   const uint32_t addr = smem_u32(bar);
   uint32_t done = 0;
   uint32_t spins = 0;
+  uint64_t t0 = 0;
   while (true) {
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
@@ -63,7 +70,15 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         : "r"(addr), "r"(parity)
         : "memory");
     if (done) break;
-    if (++spins > (1u << 26)) __trap();   // a protocol bug must fault, not hang the GPU
+    if ((++spins & 63u) == 0) {
+      const uint64_t now = globaltimer_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > 4000000000ull) {
+        printf("paci gemm: mbarrier wait timed out (tag %d, block %d, thread %d, parity %u)\n", tag, (int)blockIdx.x,
+               (int)threadIdx.x, parity);
+        __trap();
+      }
+    }
   }
 }
 __device__ __forceinline__ void tma_load_2d(void* dst, const CUtensorMap* map, uint64_t* bar, int c0, int c1) {
@@ -219,11 +234,16 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 4 * CG); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
+  // CTA pair: tcgen05.alloc.cta_group::2 must not be issued before the peer CTA is known to be running.  Without
+  // this first cluster barrier the odd CTA's alloc blocked for ever, once in ~100 launches, whenever another
+  // stream's multi-wave kernel shared the SMs (all other CTAs of the launch had finished; peer stuck in the second
+  // barrier).  The second barrier makes both allocations (and both CTAs' mbarriers) exist before the leader's
+  // first MMA writes the peer's TMEM.
+  if (CG == 2) { __syncthreads(); cluster_sync_all(); }
   if (warp == 1) {
     if (CG == 2) {
       asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
                    "r"(TMEM_COLS) : "memory");
-      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
     } else {
       asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
                    "r"(TMEM_COLS) : "memory");
@@ -232,7 +252,10 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   }
   tc_fence_before();
   __syncthreads();
-  if (CG == 2) cluster_sync_all();                       // the peer's barriers exist before anything signals them
+  if (CG == 2) {
+    cluster_sync_all();
+    if (warp == 1) asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+  }
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
@@ -252,7 +275,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const int n0 = (tile / p.tiles_m) * BLOCK_N + (int)rank * BN_CTA;
         const int kb0 = split * kb_per, kb1 = min(kb0 + kb_per, p.kb_total);
         for (int kb = kb0; kb < kb1; ++kb) {
-          mbar_wait(&empty[stage], phase ^ 1);
+          mbar_wait(&empty[stage], phase ^ 1, 1);
           uint8_t* sa = smem + stage * STAGE_BYTES;
           uint8_t* sb = sa + A_BYTES;
           const int k0 = kb * BLOCK_K;
@@ -297,11 +320,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       for (int item = worker; item < n_items; item += n_workers) {
         const int split = item % p.splits;
         const int kb0 = split * kb_per, kb1 = min(kb0 + kb_per, p.kb_total);
-        mbar_wait(&tempty[acc], acc_phase ^ 1);      // epilogue (of both CTAs) has drained this accumulator
+        mbar_wait(&tempty[acc], acc_phase ^ 1, 2);      // epilogue (of both CTAs) has drained this accumulator
         tc_fence_after();
         const uint32_t tmem_d = tmem_base + acc * BLOCK_N;
         for (int kb = kb0; kb < kb1; ++kb) {
-          mbar_wait(&full[stage], phase);
+          mbar_wait(&full[stage], phase, 3);
           tc_fence_after();
           const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES), sb = sa + A_BYTES;
 #pragma unroll
@@ -343,7 +366,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         }
         __syncwarp();
       }
-      mbar_wait(&tfull[acc], acc_phase);
+      mbar_wait(&tfull[acc], acc_phase, 4);
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BLOCK_N;
 #pragma unroll 1
@@ -406,6 +429,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     else
       asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
   }
+  if (CG == 2) cluster_sync_all();                     // pair-wide dealloc: neither CTA exits before both freed
 }
 
 // ------------------------------------------------------------------ host: tensor maps
