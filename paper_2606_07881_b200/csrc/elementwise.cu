@@ -138,95 +138,133 @@ int ln_fwd(int dtype, int rows, int D, const void* x, const void* res, const flo
 
 // =========================================================================== LayerNorm backward
 // dx = dres + rstd * (g*dy - mean(g*dy) - xhat * mean(g*dy*xhat)) with the CURRENT gain g (Eq. 1) and
-// xhat recomputed from the stashed x, mean, rstd (no parameter involved).  Each lane owns fixed
-// columns, so the column reductions Gg += sum dy*xhat, Gb += sum dy and (optionally) Gcol += sum dx
-// are register partials, combined per block through shared-memory atomics, one global atomic per
-// column per block.
+// xhat recomputed from the stashed x, mean, rstd (no parameter involved).  Two kernels, both HBM-bound:
+//   ln_bwd_dx_kernel    one warp per row, the row in registers, two warp-shuffle reductions; writes dx.
+//   ln_bwd_cols_kernel  the three column reductions Gg += sum dy*xhat, Gb += sum dy, Gcol += sum dx:
+//                       a thread owns one 16-byte column vector, a block walks its share of the rows four
+//                       at a time (independent loads in flight), the block's four row groups meet in shared
+//                       memory, then one global atomic per column per block.  It re-reads dy, x and dx, which
+//                       the first kernel has just pulled through the 126 MB L2.
+// (A single kernel holding the 3 x D/32 column partials per lane needed > 200 registers: one 8-warp CTA per
+// SM and 0.13 of HBM peak.)
 template <typename T, int NV>
-__global__ void __launch_bounds__(256) ln_bwd_kernel(int rows, int D, const T* __restrict__ dy,
-                                                     const T* __restrict__ x, const float* __restrict__ mean,
-                                                     const float* __restrict__ rstd,
-                                                     const float* __restrict__ g, const T* __restrict__ dres,
-                                                     T* __restrict__ dx, float* __restrict__ Gg,
-                                                     float* __restrict__ Gb, float* __restrict__ Gcol) {
+__global__ void __launch_bounds__(256) ln_bwd_dx_kernel(int rows, int D, const T* __restrict__ dy,
+                                                        const T* __restrict__ x, const float* __restrict__ mean,
+                                                        const float* __restrict__ rstd,
+                                                        const float* __restrict__ g, const T* __restrict__ dres,
+                                                        T* __restrict__ dx) {
   constexpr int V = Vec<T>::N;
-  extern __shared__ float sm[];  // [3][D]
   const int lane = threadIdx.x & 31;
-  const int wpb = blockDim.x >> 5;
+  const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (row >= rows) return;
   const int nvec = D / V;
-  for (int i = threadIdx.x; i < 3 * D; i += blockDim.x) sm[i] = 0.f;
-  __syncthreads();
-  float gg[NV][V], pg[NV][V], pb[NV][V], pc[NV][V];
-#pragma unroll
-  for (int i = 0; i < NV; ++i) {
-    const int c = lane + 32 * i;
-#pragma unroll
-    for (int j = 0; j < V; ++j) pg[i][j] = pb[i][j] = pc[i][j] = 0.f;
-    if (c < nvec) load_f32<V>(g + (size_t)c * V, gg[i]);
-  }
-  const float invD = 1.f / (float)D;
-  for (int row = blockIdx.x * wpb + (threadIdx.x >> 5); row < rows; row += gridDim.x * wpb) {
-    const size_t base = (size_t)row * D;
-    const float mu = mean[row], rs = rstd[row];
-    float dyv[NV][V], xh[NV][V];
-    float s1 = 0.f, s2 = 0.f;
-#pragma unroll
-    for (int i = 0; i < NV; ++i) {
-      const int c = lane + 32 * i;
-      if (c < nvec) {
-        load_vec<T>(dy + base + (size_t)c * V, dyv[i]);
-        load_vec<T>(x + base + (size_t)c * V, xh[i]);
-#pragma unroll
-        for (int j = 0; j < V; ++j) {
-          xh[i][j] = (xh[i][j] - mu) * rs;
-          pg[i][j] += dyv[i][j] * xh[i][j];
-          pb[i][j] += dyv[i][j];
-          dyv[i][j] *= gg[i][j];
-          s1 += dyv[i][j];
-          s2 += dyv[i][j] * xh[i][j];
-        }
-      }
-    }
-    s1 = warp_sum(s1) * invD;
-    s2 = warp_sum(s2) * invD;
-#pragma unroll
-    for (int i = 0; i < NV; ++i) {
-      const int c = lane + 32 * i;
-      if (c < nvec) {
-        float o[V];
-#pragma unroll
-        for (int j = 0; j < V; ++j) o[j] = rs * (dyv[i][j] - s1 - xh[i][j] * s2);
-        if (dres != nullptr) {
-          float r[V];
-          load_vec<T>(dres + base + (size_t)c * V, r);
-#pragma unroll
-          for (int j = 0; j < V; ++j) o[j] += r[j];
-        }
-        store_vec<T>(dx + base + (size_t)c * V, o);
-        if (Gcol != nullptr) {
-#pragma unroll
-          for (int j = 0; j < V; ++j) pc[i][j] += to_f(from_f<T>(o[j]));  // sum of what was stored
-        }
-      }
-    }
-  }
+  const size_t base = (size_t)row * D;
+  const float mu = mean[row], rs = rstd[row];
+  float dyv[NV][V], xh[NV][V], rv[NV][V];
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
     const int c = lane + 32 * i;
     if (c < nvec) {
+      load_vec<T>(dy + base + (size_t)c * V, dyv[i]);
+      load_vec<T>(x + base + (size_t)c * V, xh[i]);
+      if (dres != nullptr) load_vec<T>(dres + base + (size_t)c * V, rv[i]);
+    }
+  }
+  float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = lane + 32 * i;
+    if (c < nvec) {
+      float gg[V];
+      load_f32<V>(g + (size_t)c * V, gg);
 #pragma unroll
       for (int j = 0; j < V; ++j) {
-        atomicAdd(&sm[c * V + j], pg[i][j]);
-        atomicAdd(&sm[D + c * V + j], pb[i][j]);
-        if (Gcol != nullptr) atomicAdd(&sm[2 * D + c * V + j], pc[i][j]);
+        xh[i][j] = (xh[i][j] - mu) * rs;
+        dyv[i][j] *= gg[j];
+        s1 += dyv[i][j];
+        s2 += dyv[i][j] * xh[i][j];
       }
     }
   }
+  const float invD = 1.f / (float)D;
+  s1 = warp_sum(s1) * invD;
+  s2 = warp_sum(s2) * invD;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    const int c = lane + 32 * i;
+    if (c < nvec) {
+      float o[V];
+#pragma unroll
+      for (int j = 0; j < V; ++j) {
+        o[j] = rs * (dyv[i][j] - s1 - xh[i][j] * s2);
+        if (dres != nullptr) o[j] += rv[i][j];
+      }
+      store_vec<T>(dx + base + (size_t)c * V, o);
+    }
+  }
+}
+
+constexpr int LNC_TX = 128, LNC_TY = 4, LNC_U = 4;
+template <typename T>
+__global__ void __launch_bounds__(LNC_TX * LNC_TY) ln_bwd_cols_kernel(int rows, int D, const T* __restrict__ dy,
+                                                                       const T* __restrict__ x,
+                                                                       const float* __restrict__ mean,
+                                                                       const float* __restrict__ rstd,
+                                                                       const T* __restrict__ dx, float* __restrict__ Gg,
+                                                                       float* __restrict__ Gb, float* __restrict__ Gcol) {
+  constexpr int V = Vec<T>::N;
+  __shared__ float red[3][LNC_TX * V];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int c = (blockIdx.x * LNC_TX + tx) * V;
+  const bool live = c < D;
+  for (int i = ty * LNC_TX + tx; i < 3 * LNC_TX * V; i += LNC_TX * LNC_TY) (&red[0][0])[i] = 0.f;
   __syncthreads();
-  for (int i = threadIdx.x; i < D; i += blockDim.x) {
-    atomicAdd(&Gg[i], sm[i]);
-    atomicAdd(&Gb[i], sm[D + i]);
-    if (Gcol != nullptr) atomicAdd(&Gcol[i], sm[2 * D + i]);
+  float ag[V], ab[V], ac[V];
+#pragma unroll
+  for (int j = 0; j < V; ++j) ag[j] = ab[j] = ac[j] = 0.f;
+  const int stride = gridDim.y * LNC_TY;
+  if (live) {
+    for (int r0 = blockIdx.y * LNC_TY + ty; r0 < rows; r0 += LNC_U * stride) {
+      float dyv[LNC_U][V], xv[LNC_U][V], dxv[LNC_U][V], mu[LNC_U], rs[LNC_U];
+#pragma unroll
+      for (int u = 0; u < LNC_U; ++u) {
+        const int r = r0 + u * stride;
+        if (r < rows) {
+          const size_t off = (size_t)r * D + c;
+          load_vec<T>(dy + off, dyv[u]);
+          load_vec<T>(x + off, xv[u]);
+          if (Gcol != nullptr) load_vec<T>(dx + off, dxv[u]);
+          mu[u] = __ldg(mean + r);
+          rs[u] = __ldg(rstd + r);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < LNC_U; ++u) {
+        if (r0 + u * stride < rows) {
+#pragma unroll
+          for (int j = 0; j < V; ++j) {
+            ag[j] += dyv[u][j] * ((xv[u][j] - mu[u]) * rs[u]);
+            ab[j] += dyv[u][j];
+            if (Gcol != nullptr) ac[j] += dxv[u][j];
+          }
+        }
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < V; ++j) {
+      atomicAdd(&red[0][tx * V + j], ag[j]);
+      atomicAdd(&red[1][tx * V + j], ab[j]);
+      if (Gcol != nullptr) atomicAdd(&red[2][tx * V + j], ac[j]);
+    }
+  }
+  __syncthreads();
+  for (int i = ty * LNC_TX + tx; i < LNC_TX * V; i += LNC_TX * LNC_TY) {
+    const int col = blockIdx.x * LNC_TX * V + i;
+    if (col < D) {
+      atomicAdd(&Gg[col], red[0][i]);
+      atomicAdd(&Gb[col], red[1][i]);
+      if (Gcol != nullptr) atomicAdd(&Gcol[col], red[2][i]);
+    }
   }
 }
 
@@ -238,20 +276,22 @@ static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float*
   if (D % V != 0) return fail(PACI_EINVAL, "layernorm_bwd: D=%d not a multiple of %d", D, V);
   const int nv = ceil_div(D / V, 32);
   const int wpb = 8;
-  int blocks = num_sms() * 2;
-  if (blocks > ceil_div(rows, wpb)) blocks = ceil_div(rows, wpb);
-  dim3 grid(blocks), block(wpb * 32);
-  const size_t smem = 3 * (size_t)D * sizeof(float);
+  dim3 grid(ceil_div(rows, wpb)), block(wpb * 32);
 #define LNB_CASE(N)                                                                                     \
   case N:                                                                                               \
-    PACI_LAUNCH((ln_bwd_kernel<T, N>), grid, block, smem, s, rows, D, (const T*)dy, (const T*)x, mean,  \
-                rstd, g, (const T*)dres, (T*)dx, Gg, Gb, Gcol);                                         \
+    PACI_LAUNCH((ln_bwd_dx_kernel<T, N>), grid, block, 0, s, rows, D, (const T*)dy, (const T*)x, mean,  \
+                rstd, g, (const T*)dres, (T*)dx);                                                       \
     break;
   switch (nv) {
     LNB_CASE(1) LNB_CASE(2) LNB_CASE(3) LNB_CASE(4) LNB_CASE(5) LNB_CASE(6) LNB_CASE(7) LNB_CASE(8)
     default: return fail(PACI_EINVAL, "layernorm_bwd: D=%d too large", D);
   }
 #undef LNB_CASE
+  const int gx = ceil_div(D / V, LNC_TX);
+  int gy = std::max(1, num_sms() / gx);
+  gy = std::min(gy, ceil_div(rows, LNC_TY));
+  PACI_LAUNCH((ln_bwd_cols_kernel<T>), dim3(gx, gy), dim3(LNC_TX, LNC_TY), 0, s, rows, D, (const T*)dy,
+              (const T*)x, mean, rstd, (const T*)dx, Gg, Gb, Gcol);
   return PACI_OK;
 }
 
@@ -265,13 +305,21 @@ int ln_bwd(int dtype, int rows, int D, const void* dy, const void* x, const floa
 }
 
 // =========================================================================== GELU
-__device__ __forceinline__ float gelu_f(float p) {
-  const float u = GELU_C * (p + GELU_A * p * p * p);
-  return 0.5f * p * (1.f + tanhf(u));
+// tanh: accurate tanhf in fp32 mode (1e-5 parity gate); in bf16 mode the single-instruction MUFU.TANH
+// (max abs error ~5e-4, below the bf16 rounding of the result) keeps the kernels HBM-bound, not ALU-bound.
+template <typename T> __device__ __forceinline__ float tanh_t(float u) { return tanhf(u); }
+template <> __device__ __forceinline__ float tanh_t<bf16>(float u) {
+  float r;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(r) : "f"(u));
+  return r;
 }
-__device__ __forceinline__ float dgelu_f(float p) {
+template <typename T> __device__ __forceinline__ float gelu_f(float p) {
   const float u = GELU_C * (p + GELU_A * p * p * p);
-  const float th = tanhf(u);
+  return 0.5f * p * (1.f + tanh_t<T>(u));
+}
+template <typename T> __device__ __forceinline__ float dgelu_f(float p) {
+  const float u = GELU_C * (p + GELU_A * p * p * p);
+  const float th = tanh_t<T>(u);
   return 0.5f * (1.f + th) + 0.5f * p * (1.f - th * th) * GELU_C * (1.f + 3.f * GELU_A * p * p);
 }
 
@@ -282,7 +330,7 @@ __global__ void __launch_bounds__(256) gelu_fwd_kernel(size_t nvec, const T* __r
     float v[V];
     load_vec<T>(p + i * V, v);
 #pragma unroll
-    for (int j = 0; j < V; ++j) v[j] = gelu_f(v[j]);
+    for (int j = 0; j < V; ++j) v[j] = gelu_f<T>(v[j]);
     store_vec<T>(out + i * V, v);
   }
 }
@@ -299,38 +347,70 @@ int gelu_fwd(int dtype, size_t n, const void* p, void* out, cudaStream_t s) {
   return PACI_OK;
 }
 
-// Column-slab kernel shared by gelu_bwd and colsum: thread owns one 16-byte column vector, the
-// block loops over rows (grid.y splits the rows), partial column sums stay in registers and end in
-// one global atomic per column per block.
+// Column-slab kernel shared by gelu_bwd and colsum: a thread owns one 16-byte column vector, a block of
+// CS_TX x CS_TY threads walks its share of the rows four at a time (independent 16-byte loads in flight),
+// partial column sums stay in registers, the block's CS_TY row groups meet in shared memory, and the block
+// ends with ONE vector atomic (red.global.add.v4.f32) per 4 columns.  (One scalar atomic per column per
+// 128-thread block put ~3000 serialized L2 atomics on every 32-byte sector of G: 0.15 of HBM peak.)
+constexpr int CS_TX = 64, CS_TY = 8, CS_U = 4;
+__device__ __forceinline__ void red_add_v4(float* dst, float a, float b, float c, float d) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
 template <typename T, bool GELU>
-__global__ void __launch_bounds__(256) colslab_kernel(int rows, int cols, const T* __restrict__ a,
-                                                      const T* __restrict__ p, T* __restrict__ out,
-                                                      float* __restrict__ G) {
+__global__ void __launch_bounds__(CS_TX * CS_TY) colslab_kernel(int rows, int cols, const T* __restrict__ a,
+                                                                 const T* __restrict__ p, T* __restrict__ out,
+                                                                 float* __restrict__ G) {
   constexpr int V = Vec<T>::N;
-  const int c = (blockIdx.x * blockDim.x + threadIdx.x) * V;
-  if (c >= cols) return;
+  __shared__ __align__(16) float red[CS_TX * V];
+  const int tx = threadIdx.x, ty = threadIdx.y;
+  const int c = (blockIdx.x * CS_TX + tx) * V;
+  const bool live = c < cols;
+  if (G != nullptr) {
+    for (int i = ty * CS_TX + tx; i < CS_TX * V; i += CS_TX * CS_TY) red[i] = 0.f;
+    __syncthreads();
+  }
   float acc[V];
 #pragma unroll
   for (int j = 0; j < V; ++j) acc[j] = 0.f;
-  for (int r = blockIdx.y; r < rows; r += gridDim.y) {
-    const size_t off = (size_t)r * cols + c;
-    float v[V];
-    load_vec<T>(a + off, v);
-    if (GELU) {
-      float pv[V];
-      load_vec<T>(p + off, pv);
+  const int stride = gridDim.y * CS_TY;
+  if (live) {
+    for (int r0 = blockIdx.y * CS_TY + ty; r0 < rows; r0 += CS_U * stride) {
+      float v[CS_U][V], pv[CS_U][V];
 #pragma unroll
-      for (int j = 0; j < V; ++j) v[j] *= dgelu_f(pv[j]);
-      store_vec<T>(out + off, v);
+      for (int u = 0; u < CS_U; ++u) {
+        const int r = r0 + u * stride;
+        if (r < rows) {
+          const size_t off = (size_t)r * cols + c;
+          load_vec<T>(a + off, v[u]);
+          if (GELU) load_vec<T>(p + off, pv[u]);
+        }
+      }
 #pragma unroll
-      for (int j = 0; j < V; ++j) v[j] = to_f(from_f<T>(v[j]));  // sum what was stored
+      for (int u = 0; u < CS_U; ++u) {
+        const int r = r0 + u * stride;
+        if (r < rows) {
+          if (GELU) {
+#pragma unroll
+            for (int j = 0; j < V; ++j) v[u][j] *= dgelu_f<T>(pv[u][j]);
+            store_vec<T>(out + (size_t)r * cols + c, v[u]);
+#pragma unroll
+            for (int j = 0; j < V; ++j) v[u][j] = to_f(from_f<T>(v[u][j]));  // sum what was stored
+          }
+#pragma unroll
+          for (int j = 0; j < V; ++j) acc[j] += v[u][j];
+        }
+      }
     }
-#pragma unroll
-    for (int j = 0; j < V; ++j) acc[j] += v[j];
   }
-  if (G != nullptr) {
+  if (G == nullptr) return;
+  if (live) {
 #pragma unroll
-    for (int j = 0; j < V; ++j) atomicAdd(&G[c + j], acc[j]);
+    for (int j = 0; j < V; ++j) atomicAdd(&red[tx * V + j], acc[j]);
+  }
+  __syncthreads();
+  for (int i = (ty * CS_TX + tx) * 4; i < CS_TX * V; i += CS_TX * CS_TY * 4) {
+    const int col = blockIdx.x * CS_TX * V + i;
+    if (col < cols) red_add_v4(G + col, red[i], red[i + 1], red[i + 2], red[i + 3]);   // cols % 4 == 0
   }
 }
 
@@ -340,16 +420,16 @@ static int colslab(int dtype, int rows, int cols, const void* a, const void* p, 
   if (rows <= 0 || cols <= 0) return PACI_OK;
   const int V = dtype == PACI_BF16 ? 8 : 4;
   if (cols % V) return fail(PACI_EINVAL, "colslab: cols=%d not a multiple of %d", cols, V);
-  const int threads = 128;
-  const int gx = ceil_div(cols / V, threads);
-  int gy = std::max(1, num_sms() * 8 / gx);
-  if (gy > rows) gy = rows;
-  dim3 grid(gx, gy);
+  if (G != nullptr && (uintptr_t)G % 16) return fail(PACI_EINVAL, "colslab: G not 16-byte aligned");
+  const int gx = ceil_div(cols / V, CS_TX);
+  int gy = std::max(1, num_sms() * 4 / gx);
+  gy = std::min(gy, ceil_div(rows, CS_TY));
+  dim3 grid(gx, gy), block(CS_TX, CS_TY);
   if (dtype == PACI_BF16)
-    PACI_LAUNCH((colslab_kernel<bf16, GELU>), grid, threads, 0, s, rows, cols, (const bf16*)a, (const bf16*)p,
+    PACI_LAUNCH((colslab_kernel<bf16, GELU>), grid, block, 0, s, rows, cols, (const bf16*)a, (const bf16*)p,
                 (bf16*)out, G);
   else
-    PACI_LAUNCH((colslab_kernel<float, GELU>), grid, threads, 0, s, rows, cols, (const float*)a,
+    PACI_LAUNCH((colslab_kernel<float, GELU>), grid, block, 0, s, rows, cols, (const float*)a,
                 (const float*)p, (float*)out, G);
   return PACI_OK;
 }
