@@ -22,6 +22,11 @@ static bool attn_backend_tensor() {
   static const bool simt = env_is("PACI_ATTN", "simt");
   return !simt;
 }
+// PACI_ATTN=mma keeps the warp-level mma.sync kernels even where the tcgen05 kernels apply (T % 128 == 0)
+static bool attn_backend_tcgen05() {
+  static const bool off = env_is("PACI_ATTN", "mma") || env_is("PACI_ATTN", "simt");
+  return !off;
+}
 
 int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
          const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s) {
@@ -34,6 +39,7 @@ int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, con
 }
 
 int attention_fwd_mma(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
+int attention_fwd_tc(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
 int attention_bwd_mma(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
                       void* dqkv, float* scratch, cudaStream_t s);
 size_t attention_bwd_mma_scratch_bytes(int mu, int T, int H);
@@ -44,6 +50,7 @@ int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void
   ProfScope prof(PC_ATTN_FWD, 2.0 * mu * H * (double)T * T * dh, e * 4.0 * nd + 4.0 * mu * H * T, s);
   if (dtype == PACI_BF16 && attn_backend_tensor()) {
     if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
+    if (T % 128 == 0 && attn_backend_tcgen05()) return attention_fwd_tc(mu, T, H, qkv, o, lse, s);
     return attention_fwd_mma(mu, T, H, qkv, o, lse, s);
   }
   return attention_fwd_simt(dtype, mu, T, H, dh, qkv, o, lse, s);
