@@ -245,7 +245,290 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
   }
 }
 
+// ============================================================================== backward
+// Two launches of ONE kernel template (deterministic, no atomics), both with this skeleton: two STATIONARY
+// 128-row tiles X0, X1 and a stream of 64-row tile pairs Y0, Y1 (2-stage TMA ring); per step
+//     T0 = X0 Y0^T,  T1 = X1 Y1^T            (M128 N64 K64, into TMEM)
+//     E0, E1 = elementwise(T0, T1)           (thread = TMEM lane = stationary row; bf16 into swizzled smem)
+//     ACC0 += E0 Y1,  ACC1 += E1 Y0          (M128 N64 K64, TMEM accumulators across all steps)
+//   DKDV (one CTA per 128-key block): X = K_j, V_j; Y = Q_i, dO_i over the query steps at or below the
+//        diagonal.  T0 = S^T, T1 = dP^T, E0 = P^T, E1 = dS^T; ACC0 = dV = P^T dO, ACC1 = dK = dS^T Q.
+//        lse and delta are indexed by the streamed (query) index: 2 x 256 B per step ride the same ring.
+//   DQ   (one CTA per 128-query tile): X = Q_i, dO_i; Y = K_j, V_j over the key steps at or left of the
+//        diagonal.  T0 = S, T1 = dP, E1 = dS; ACC1 = dQ = dS K.  lse, delta are per-thread scalars.
+// with P = exp2(S c - lse log2e), dS = P o (dP - delta) / sqrt(dh); the probabilities are recomputed from the
+// stashed q, k and lse -- no parameter is involved, so this is not the checkpointed variant of P:282.
+// T_{t+1} is issued before ACC_t, so the tensor pipe computes the next scores while the 128 elementwise
+// threads work; two CTAs (96 KB smem, 256 TMEM columns each) share an SM.
+constexpr int BWD_THREADS = 192;
+constexpr uint32_t HALF_BYTES = 64 * 128;               // 64 rows x 64 bf16
+constexpr uint32_t BWD_SMEM = 2 * TILE_BYTES + 2 * (2 * HALF_BYTES) + 2 * TILE_BYTES + 2 * 512 + 256;
+
+__device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+template <bool DKDV>
+__global__ void __launch_bounds__(BWD_THREADS, 2)
+attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constant__ CUtensorMap mX1,
+                   const __grid_constant__ CUtensorMap mY0, const __grid_constant__ CUtensorMap mY1, int T, int H,
+                   const float* __restrict__ lse, const float* __restrict__ delta, bf16* __restrict__ dqkv) {
+  extern __shared__ __align__(1024) uint8_t smem[];
+  constexpr uint32_t YST = 2 * HALF_BYTES;               // one ring stage: Y0, Y1 (1024-byte aligned tiles)
+  uint8_t* sX0 = smem;
+  uint8_t* sX1 = sX0 + TILE_BYTES;
+  uint8_t* sY = sX1 + TILE_BYTES;
+  uint8_t* sE0 = sY + 2 * YST;
+  uint8_t* sE1 = sE0 + TILE_BYTES;
+  uint8_t* sStat = sE1 + TILE_BYTES;                     // per stage: lse[64], delta[64] of the streamed rows
+  uint64_t* bars = (uint64_t*)(sStat + 2 * 512);
+  uint64_t *x_full = bars, *y_full = bars + 1, *y_empty = bars + 3, *t_full = bars + 5, *e_full = bars + 6,
+           *e_empty = bars + 7, *acc_full = bars + 8;
+  uint32_t* tmem_slot = (uint32_t*)(bars + 9);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int D = H * DH;
+  const int nt = T / 128;
+  const int per = H * (int)(gridDim.x / (nt * H));       // H * mu
+  const int rank = (int)blockIdx.x / per;                // heaviest tiles first
+  const int tile = DKDV ? rank : nt - 1 - rank;
+  const int rem = (int)blockIdx.x % per;
+  const int h = rem % H, b = rem / H;
+  const int x0 = tile * 128;                             // first stationary row (key for DKDV, query for DQ)
+  const int c_begin = DKDV ? x0 : 0;                     // streamed rows [c_begin, c_end), 64 per step
+  const int c_end = DKDV ? T : x0 + 128;
+  const int n_steps = (c_end - c_begin) / 64;
+  const int row0 = b * T;
+
+  if ((smem_u32(smem) & 1023u) != 0) __trap();
+  if (threadIdx.x == 0) {
+    mbar_init(x_full, 1);
+    for (int i = 0; i < 2; ++i) { mbar_init(&y_full[i], 1); mbar_init(&y_empty[i], 1); }
+    mbar_init(t_full, 1); mbar_init(e_full, 128); mbar_init(e_empty, 1); mbar_init(acc_full, 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(256) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+  const uint32_t tT0 = tmem_base, tT1 = tmem_base + 64, tA0 = tmem_base + 128, tA1 = tmem_base + 192;
+
+  if (warp == 0) {
+    if (lane == 0) {
+      // column of each operand inside its tensor: qkv = [q | k | v], dO = [D]
+      const int cx0 = DKDV ? D + h * DH : h * DH;        // K_j | Q_i
+      const int cx1 = DKDV ? 2 * D + h * DH : h * DH;    // V_j | dO_i
+      const int cy0 = DKDV ? h * DH : D + h * DH;        // Q   | K
+      const int cy1 = DKDV ? h * DH : 2 * D + h * DH;    // dO  | V
+      mbar_expect_tx(x_full, 2 * TILE_BYTES);
+      tma_load_2d(sX0, &mX0, x_full, cx0, row0 + x0);
+      tma_load_2d(sX1, &mX1, x_full, cx1, row0 + x0);
+      const float* lrow = lse + ((size_t)b * H + h) * T;
+      const float* drow = delta + ((size_t)b * H + h) * T;
+      for (int t = 0; t < n_steps; ++t) {
+        const int st = t & 1, c0 = c_begin + t * 64;
+        mbar_wait(&y_empty[st], ((uint32_t)(t >> 1) & 1u) ^ 1u, 21);
+        uint8_t* y = sY + st * YST;
+        mbar_expect_tx(&y_full[st], 2 * HALF_BYTES + (DKDV ? 512u : 0u));
+        tma_load_2d(y, &mY0, &y_full[st], cy0, row0 + c0);
+        tma_load_2d(y + HALF_BYTES, &mY1, &y_full[st], cy1, row0 + c0);
+        if (DKDV) {
+          bulk_load_1d(sStat + st * 512, lrow + c0, 256, &y_full[st]);
+          bulk_load_1d(sStat + st * 512 + 256, drow + c0, 256, &y_full[st]);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    if (lane == 0) {
+      constexpr uint32_t ID_T = idesc(128, 64, false, false), ID_ACC = idesc(128, 64, false, true);
+      const uint32_t aX0 = smem_u32(sX0), aX1 = smem_u32(sX1), aE0 = smem_u32(sE0), aE1 = smem_u32(sE1);
+      auto issue_t = [&](int t) {
+        const int st = t & 1;
+        mbar_wait(&y_full[st], (uint32_t)(t >> 1) & 1u, 22);
+        tc_fence_after();
+        const uint32_t aY0 = smem_u32(sY + st * YST), aY1 = aY0 + HALF_BYTES;
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)
+          umma_bf16(tT0, smem_desc(aX0 + kk * 32, 16, 1024), smem_desc(aY0 + kk * 32, 16, 1024), ID_T, kk > 0 ? 1u : 0u);
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)
+          umma_bf16(tT1, smem_desc(aX1 + kk * 32, 16, 1024), smem_desc(aY1 + kk * 32, 16, 1024), ID_T, kk > 0 ? 1u : 0u);
+        umma_commit(t_full);
+      };
+      mbar_wait(x_full, 0, 23);
+      issue_t(0);
+      for (int t = 0; t < n_steps; ++t) {
+        mbar_wait(e_full, (uint32_t)t & 1u, 24);          // E_t is in shared memory and T_t has been consumed
+        tc_fence_after();
+        if (t + 1 < n_steps) issue_t(t + 1);
+        const int st = t & 1;
+        const uint32_t aY0 = smem_u32(sY + st * YST), aY1 = aY0 + HALF_BYTES;
+        const uint32_t acc = t > 0 ? 1u : 0u;
+        if (DKDV) {
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk)                  // dV += P^T dO
+            umma_bf16(tA0, smem_desc(aE0 + kk * 32, 16, 1024), smem_desc(aY1 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
+        }
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk)                    // dK += dS^T Q   |   dQ += dS K
+          umma_bf16(tA1, smem_desc(aE1 + kk * 32, 16, 1024), smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
+        umma_commit(&y_empty[st]);
+        umma_commit(e_empty);
+      }
+      umma_commit(acc_full);
+    }
+  } else {
+    const int r = (warp & 3) * 32 + lane;                 // stationary row inside the tile = TMEM lane
+    const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
+    const float c = rsqrtf((float)DH) * LOG2E, inv_sqrt = rsqrtf((float)DH);
+    float my_lse2 = 0.f, my_delta = 0.f;
+    if (!DKDV) {
+      my_lse2 = lse[((size_t)b * H + h) * T + x0 + r] * LOG2E;
+      my_delta = delta[((size_t)b * H + h) * T + x0 + r];
+    }
+    uint8_t* e0row = sE0 + r * 128;
+    uint8_t* e1row = sE1 + r * 128;
+    for (int t = 0; t < n_steps; ++t) {
+      const int st = t & 1, c0 = c_begin + t * 64;
+      mbar_wait(t_full, (uint32_t)t & 1u, 25);
+      tc_fence_after();
+      uint32_t s[64], dp[64];
+      tmem_ld32_nowait(tT0 + lane_off, s);
+      tmem_ld32_nowait(tT0 + lane_off + 32, s + 32);
+      tmem_ld32_nowait(tT1 + lane_off, dp);
+      tmem_ld32_nowait(tT1 + lane_off + 32, dp + 32);
+      tmem_ld_wait();
+      const float* st_lse = reinterpret_cast<const float*>(sStat + st * 512);
+      const float* st_del = st_lse + 64;
+      if (DKDV) mbar_wait(&y_full[st], (uint32_t)(t >> 1) & 1u, 26);   // the step's lse / delta have landed
+      // causal keep: query >= key.  DKDV: query = c0 + i, key = x0 + r.  DQ: query = x0 + r, key = c0 + i.
+      const bool diag = DKDV ? (c0 < x0 + 128) : (c0 + 63 > x0);
+      if (t > 0) mbar_wait(e_empty, (uint32_t)(t - 1) & 1u, 27);        // ACC_{t-1} has finished reading E
+#pragma unroll
+      for (int ch = 0; ch < 8; ++ch) {
+        uint32_t wp[4], wd[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          float pv[2], dv[2];
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int i = ch * 8 + 2 * u + e;
+            const float l2 = DKDV ? st_lse[i] * LOG2E : my_lse2;
+            const float dl = DKDV ? st_del[i] : my_delta;
+            float p = ex2(__uint_as_float(s[i]) * c - l2);
+            if (diag) {
+              const bool keep = DKDV ? (c0 + i >= x0 + r) : (x0 + r >= c0 + i);
+              p = keep ? p : 0.f;
+            }
+            pv[e] = p;
+            dv[e] = p * (__uint_as_float(dp[i]) - dl) * inv_sqrt;
+          }
+          wp[u] = pack_bf16x2(pv[0], pv[1]);
+          wd[u] = pack_bf16x2(dv[0], dv[1]);
+        }
+        const uint32_t off = (uint32_t)((ch ^ (r & 7)) << 4);
+        if (DKDV) sts128(e0row + off, wp[0], wp[1], wp[2], wp[3]);
+        sts128(e1row + off, wd[0], wd[1], wd[2], wd[3]);
+      }
+      fence_async_smem();
+      tc_fence_before();
+      mbar_arrive(e_full);
+    }
+    // epilogue: accumulators -> bf16 rows of dqkv
+    mbar_wait(acc_full, 0, 28);
+    tc_fence_after();
+    bf16* orow = dqkv + ((size_t)row0 + x0 + r) * 3 * D + h * DH;
+    auto store_acc = [&](uint32_t taddr, bf16* dst) {
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        uint32_t ov[32];
+        tmem_ld32(taddr + lane_off + q * 32, ov);
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          uint4 w;
+          w.x = pack_bf16x2(__uint_as_float(ov[8 * i]), __uint_as_float(ov[8 * i + 1]));
+          w.y = pack_bf16x2(__uint_as_float(ov[8 * i + 2]), __uint_as_float(ov[8 * i + 3]));
+          w.z = pack_bf16x2(__uint_as_float(ov[8 * i + 4]), __uint_as_float(ov[8 * i + 5]));
+          w.w = pack_bf16x2(__uint_as_float(ov[8 * i + 6]), __uint_as_float(ov[8 * i + 7]));
+          *reinterpret_cast<uint4*>(dst + q * 32 + i * 8) = w;
+        }
+      }
+    };
+    if (DKDV) {
+      store_acc(tA0, orow + 2 * D);   // dV
+      store_acc(tA1, orow + D);       // dK
+    } else {
+      store_acc(tA1, orow);           // dQ
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(256) : "memory");
+  }
+}
+
+
+// delta[b,h,t] = sum_d dO[b,t,h,d] * O[b,t,h,d]: 8 threads per (b,t,h), one 16-byte vector each
+__global__ void __launch_bounds__(256) attn_delta_tc_kernel(size_t n_vec, int T, int H, const bf16* __restrict__ dout,
+                                                            const bf16* __restrict__ o, float* __restrict__ delta) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  float acc = 0.f;
+  if (i < n_vec) {
+    float a[8], c[8];
+    load_vec<bf16>(dout + i * 8, a);
+    load_vec<bf16>(o + i * 8, c);
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc += a[j] * c[j];
+  }
+#pragma unroll
+  for (int sh = 1; sh < 8; sh <<= 1) acc += __shfl_xor_sync(0xffffffffu, acc, sh);
+  if (i < n_vec && (threadIdx.x & 7) == 0) {
+    const size_t hv = i >> 3;                  // (b*T + t)*H + h
+    const size_t bt = hv / H;
+    delta[((bt / T) * H + hv % H) * T + bt % T] = acc;
+  }
+}
+
 }  // namespace
+
+size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H) { return (size_t)mu * H * T * sizeof(float); }
+
+int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
+                     void* dqkv, float* scratch, cudaStream_t s) {
+  const int D = H * DH;
+  const uint64_t rows = (uint64_t)mu * T;
+  CUtensorMap q128, q64, d128, d64;
+  int rc;
+  if ((rc = make_tensor_map(&q128, qkv, 3 * (uint64_t)D, rows, 3 * (uint64_t)D, 64, 128, 2))) return rc;
+  if ((rc = make_tensor_map(&q64, qkv, 3 * (uint64_t)D, rows, 3 * (uint64_t)D, 64, 64, 2))) return rc;
+  if ((rc = make_tensor_map(&d128, dout, (uint64_t)D, rows, (uint64_t)D, 64, 128, 2))) return rc;
+  if ((rc = make_tensor_map(&d64, dout, (uint64_t)D, rows, (uint64_t)D, 64, 64, 2))) return rc;
+  static bool attr_set = false;
+  if (!attr_set) {
+    PACI_CUDA_OK(cudaFuncSetAttribute(attn_bwd_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BWD_SMEM));
+    PACI_CUDA_OK(cudaFuncSetAttribute(attn_bwd_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BWD_SMEM));
+    attr_set = true;
+  }
+  float* delta = scratch;
+  const size_t n_vec = (size_t)mu * T * D / 8;
+  PACI_LAUNCH(attn_delta_tc_kernel, ceil_div((long long)n_vec, 256), 256, 0, s, n_vec, T, H, (const bf16*)dout,
+              (const bf16*)o, delta);
+  const int grid = (T / 128) * H * mu;
+  // dK, dV: stationary K_j, V_j (qkv, 128-row boxes); streamed Q_i (qkv), dO_i (dout), 64-row boxes
+  PACI_LAUNCH(attn_bwd_tc_kernel<true>, grid, BWD_THREADS, BWD_SMEM, s, q128, q128, q64, d64, T, H, lse, delta,
+              (bf16*)dqkv);
+  // dQ: stationary Q_i (qkv), dO_i (dout); streamed K_j, V_j (qkv)
+  PACI_LAUNCH(attn_bwd_tc_kernel<false>, grid, BWD_THREADS, BWD_SMEM, s, q128, d128, q64, q64, T, H, lse, delta,
+              (bf16*)dqkv);
+  return PACI_OK;
+}
 
 int attention_fwd_tc(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s) {
   const int D = H * DH;

@@ -40,6 +40,8 @@ int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, con
 
 int attention_fwd_mma(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
 int attention_fwd_tc(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
+int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
+                     void* dqkv, float* scratch, cudaStream_t s);
 int attention_bwd_mma(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
                       void* dqkv, float* scratch, cudaStream_t s);
 size_t attention_bwd_mma_scratch_bytes(int mu, int T, int H);
@@ -62,6 +64,7 @@ int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, con
   ProfScope prof(PC_ATTN_BWD, 4.0 * mu * H * (double)T * T * dh, e * 8.0 * nd + 4.0 * mu * H * T, s);
   if (dtype == PACI_BF16 && attn_backend_tensor()) {
     if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
+    if (T % 128 == 0 && attn_backend_tcgen05()) return attention_bwd_tc(mu, T, H, dout, qkv, o, lse, dqkv, scratch, s);
     return attention_bwd_mma(mu, T, H, dout, qkv, o, lse, dqkv, scratch, s);
   }
   return attention_bwd_simt(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, s);
