@@ -108,6 +108,7 @@ struct ProfScope {   // counts the launch; every stride-th one is timed with eve
   int idx_;
   cudaStream_t stream_;
 };
+void prof_set_peer_streams(const cudaStream_t* streams, int n);   // sampled launches run alone w.r.t. these
 int stage_cfg_field(const ::paci_stage* st, int field);   // i-th int32 of the stage's paci_stage_config
 
 // ---------------------------------------------------------------- kernel launchers (host)

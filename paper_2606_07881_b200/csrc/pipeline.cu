@@ -149,6 +149,10 @@ int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_
   for (int s = 0; s < S; ++s) v0[s] = paci_version(p->st[s]);
   const int64_t launches0 = paci_launch_count();
 
+  struct PeerGuard {   // sampled launches of the in-library profiler run exclusively w.r.t. the stage streams
+    explicit PeerGuard(const std::vector<cudaStream_t>& v) { prof_set_peer_streams(v.data(), (int)v.size()); }
+    ~PeerGuard() { prof_set_peer_streams(nullptr, 0); }
+  } peer_guard(p->streams);
   // all stage streams start after ev_start
   PACI_CUDA_OK(cudaEventRecord(p->ev_start, p->main));
   for (int s = 0; s < S; ++s) PACI_CUDA_OK(cudaStreamWaitEvent(p->streams[s], p->ev_start, 0));

@@ -3,6 +3,13 @@
 // bytes).  All launches are counted; every `stride`-th one is bracketed by a pair of CUDA events
 // recorded on the stream the kernel is launched on, so the measurement lives inside the timed
 // region of the benchmark at negligible cost.  Host code only.
+//
+// Exclusive samples.  The schedule driver runs the S emulated stages on S streams, so a kernel bracketed
+// by events on its own stream shares the SMs with the other stages' kernels and its event time is a
+// latency under contention, not its own duration.  While a pipeline run is active (prof_set_peer_streams)
+// a SAMPLED launch therefore first waits for everything already queued on the other stage streams, and
+// those streams wait for the sample's end event: the sampled kernel runs alone, with the caches and clocks
+// of the real step, and 1 launch in `stride` pays for it.
 #include <mutex>
 #include <vector>
 
@@ -19,6 +26,7 @@ paci_prof_entry g_tot[PACI_PROF_NCAT];
 std::vector<Sample> g_samples;
 std::vector<cudaEvent_t> g_pool;
 size_t g_pool_used = 0;
+std::vector<cudaStream_t> g_peers;
 
 cudaEvent_t take_event() {
   if (g_pool_used == g_pool.size()) {
@@ -41,6 +49,11 @@ ProfScope::ProfScope(int cat, double flops, double bytes, cudaStream_t s) : idx_
   if (g_counter++ % g_stride != 0) return;
   Sample smp{cat, flops, bytes, take_event(), take_event()};
   if (!smp.e0 || !smp.e1) return;
+  for (cudaStream_t peer : g_peers) {
+    if (peer == s) continue;
+    cudaEvent_t e = take_event();
+    if (!e || cudaEventRecord(e, peer) != cudaSuccess || cudaStreamWaitEvent(s, e, 0) != cudaSuccess) return;
+  }
   if (cudaEventRecord(smp.e0, s) != cudaSuccess) return;
   g_samples.push_back(smp);
   idx_ = (int)g_samples.size() - 1;
@@ -49,6 +62,13 @@ ProfScope::~ProfScope() {
   if (idx_ < 0) return;
   std::lock_guard<std::mutex> g(g_mu);
   cudaEventRecord(g_samples[idx_].e1, stream_);
+  for (cudaStream_t peer : g_peers)
+    if (peer != stream_) cudaStreamWaitEvent(peer, g_samples[idx_].e1, 0);
+}
+
+void prof_set_peer_streams(const cudaStream_t* streams, int n) {
+  std::lock_guard<std::mutex> g(g_mu);
+  g_peers.assign(streams, streams + (streams ? n : 0));
 }
 
 }  // namespace paci
