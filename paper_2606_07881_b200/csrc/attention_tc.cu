@@ -14,6 +14,8 @@
 //              max has grown by more than 2^8 since the reference max m_ref was taken ("lazy rescale"): the
 //              final O / l and lse = m_ref + log2 l do not depend on which reference was used.
 // qkv is packed [mu, T, 3D]: q | k | v, head h at columns h*64 .. h*64+63 (R17).
+#include <type_traits>
+
 #include "tc_ptx.cuh"
 
 namespace paci {
@@ -37,6 +39,22 @@ __device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t* r) {
         "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
       : "r"(taddr));
 }
+__device__ __forceinline__ void tmem_ld16_nowait(uint32_t taddr, uint32_t* r) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+        "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr));
+}
+template <int N> __device__ __forceinline__ void tmem_ld_cols_nowait(uint32_t taddr, uint32_t* r) {
+  static_assert(N == 16 || N == 32 || N == 64, "column count");
+  if constexpr (N == 16) tmem_ld16_nowait(taddr, r);
+  else {
+#pragma unroll
+    for (int q = 0; q < N / 32; ++q) tmem_ld32_nowait(taddr + q * 32, r + q * 32);
+  }
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
   asm volatile(
@@ -54,6 +72,35 @@ __device__ __forceinline__ float ex2(float x) {
   float r;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
   return r;
+}
+
+// mbarrier wait for the 128..256 elementwise threads: after a few failed polls they sleep between polls, so
+// waiting warps do not take issue slots from the working warps of the other CTA on the SM.
+__device__ __forceinline__ void mbar_wait_many(uint64_t* bar, uint32_t parity, int tag) {
+  const uint32_t addr = smem_u32(bar);
+  for (int i = 0; i < 4; ++i) {
+    uint32_t done;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.b32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    if (done) return;
+  }
+  uint32_t spins = 0;
+  uint64_t t0 = 0;
+  while (true) {
+    uint32_t done;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.b32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    if (done) return;
+    __nanosleep(64);
+    if ((++spins & 255u) == 0) {
+      const uint64_t now = globaltimer_ns();
+      if (t0 == 0) t0 = now;
+      else if (now - t0 > 4000000000ull) {
+        printf("paci attention: mbarrier wait timed out (tag %d, block %d, thread %d)\n", tag, (int)blockIdx.x, (int)threadIdx.x);
+        __trap();
+      }
+    }
+  }
 }
 
 // instruction descriptor: D fp32, A/B bf16, majors, N>>3 at bit 17, M>>4 at bit 24
@@ -164,7 +211,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
     float m_ref = -INFINITY, l = 0.f;
     uint8_t* prow = sP + r * 128;
     for (int j = 0; j < n_kb; ++j) {
-      mbar_wait(s_full, (uint32_t)j & 1u, 17);
+      mbar_wait_many(s_full, (uint32_t)j & 1u, 17);
       tc_fence_after();
       uint32_t s[128];
 #pragma unroll
@@ -186,7 +233,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
       } else if (__any_sync(0xffffffffu, grow)) {
         const float f = grow ? ex2(m_ref - mx) : 1.f;
         if (grow) { m_ref = mx; l *= f; }
-        mbar_wait(o_full, (uint32_t)(j - 1) & 1u, 18);     // P_{j-1} V_{j-1} (and everything before) is in TMEM
+        mbar_wait_many(o_full, (uint32_t)(j - 1) & 1u, 18);     // P_{j-1} V_{j-1} (and everything before) is in TMEM
         tc_fence_after();
 #pragma unroll
         for (int q = 0; q < 2; ++q) {
@@ -217,7 +264,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
       mbar_arrive(p_full);
     }
     // epilogue: O / l -> bf16, lse
-    mbar_wait(o_full, (uint32_t)(n_kb - 1) & 1u, 19);
+    mbar_wait_many(o_full, (uint32_t)(n_kb - 1) & 1u, 19);
     tc_fence_after();
     const float inv = 1.f / l;
     bf16* orow = o + ((size_t)b * T + q0 + r) * D + h * DH;
@@ -260,17 +307,22 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
 // stashed q, k and lse -- no parameter is involved, so this is not the checkpointed variant of P:282.
 // T_{t+1} is issued before ACC_t, so the tensor pipe computes the next scores while the 128 elementwise
 // threads work; two CTAs (96 KB smem, 256 TMEM columns each) share an SM.
-constexpr int BWD_THREADS = 192;
+constexpr int BWD_EW = 2;                               // elementwise warpgroups: each thread owns 64/EW columns
+constexpr int BWD_THREADS = 64 + 128 * BWD_EW;
 constexpr uint32_t HALF_BYTES = 64 * 128;               // 64 rows x 64 bf16
-constexpr uint32_t BWD_SMEM = 2 * TILE_BYTES + 2 * (2 * HALF_BYTES) + 2 * TILE_BYTES + 2 * 512 + 256;
+// ring depth: DKDV needs both E tiles (P^T, dS^T) and fits 2 stages in half an SM's shared memory; DQ has one E tile and takes 3
+__host__ __device__ constexpr int bwd_stages(bool dkdv) { return dkdv ? 2 : 3; }
+__host__ __device__ constexpr uint32_t bwd_smem(bool dkdv) {
+  return 2 * TILE_BYTES + bwd_stages(dkdv) * (2 * HALF_BYTES + 512) + (dkdv ? 2u : 1u) * TILE_BYTES + 256;
+}
 
 __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-template <bool DKDV>
-__global__ void __launch_bounds__(BWD_THREADS, 2)
+template <bool DKDV, int EW>
+__global__ void __launch_bounds__(64 + 128 * EW, 2)
 attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constant__ CUtensorMap mX1,
                    const __grid_constant__ CUtensorMap mY0, const __grid_constant__ CUtensorMap mY1, int T, int H,
                    const float* __restrict__ lse, const float* __restrict__ delta, bf16* __restrict__ dqkv) {
@@ -279,13 +331,14 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   uint8_t* sX0 = smem;
   uint8_t* sX1 = sX0 + TILE_BYTES;
   uint8_t* sY = sX1 + TILE_BYTES;
-  uint8_t* sE0 = sY + 2 * YST;
-  uint8_t* sE1 = sE0 + TILE_BYTES;
-  uint8_t* sStat = sE1 + TILE_BYTES;                     // per stage: lse[64], delta[64] of the streamed rows
-  uint64_t* bars = (uint64_t*)(sStat + 2 * 512);
-  uint64_t *x_full = bars, *y_full = bars + 1, *y_empty = bars + 3, *t_full = bars + 5, *e_full = bars + 6,
-           *e_empty = bars + 7, *acc_full = bars + 8;
-  uint32_t* tmem_slot = (uint32_t*)(bars + 9);
+  constexpr int NST = bwd_stages(DKDV);
+  uint8_t* sE1 = sY + NST * YST;
+  uint8_t* sE0 = sE1 + TILE_BYTES;                       // DKDV only
+  uint8_t* sStat = sE1 + (DKDV ? 2 : 1) * TILE_BYTES;    // per stage: lse2[64], delta[64] of the streamed rows
+  uint64_t* bars = (uint64_t*)(sStat + NST * 512);
+  uint64_t *x_full = bars, *y_full = bars + 1, *y_empty = bars + 1 + NST, *t_full = bars + 1 + 2 * NST, *e_full = t_full + 1,
+           *e_empty = t_full + 2, *acc_full = t_full + 3;
+  uint32_t* tmem_slot = (uint32_t*)(t_full + 4);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int D = H * DH;
@@ -304,8 +357,8 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   if ((smem_u32(smem) & 1023u) != 0) __trap();
   if (threadIdx.x == 0) {
     mbar_init(x_full, 1);
-    for (int i = 0; i < 2; ++i) { mbar_init(&y_full[i], 1); mbar_init(&y_empty[i], 1); }
-    mbar_init(t_full, 1); mbar_init(e_full, 128); mbar_init(e_empty, 1); mbar_init(acc_full, 1);
+    for (int i = 0; i < NST; ++i) { mbar_init(&y_full[i], 1); mbar_init(&y_empty[i], 1); }
+    mbar_init(t_full, 1); mbar_init(e_full, 128 * EW); mbar_init(e_empty, 1); mbar_init(acc_full, 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -331,8 +384,8 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       const float* lrow = lse + ((size_t)b * H + h) * T;
       const float* drow = delta + ((size_t)b * H + h) * T;
       for (int t = 0; t < n_steps; ++t) {
-        const int st = t & 1, c0 = c_begin + t * 64;
-        mbar_wait(&y_empty[st], ((uint32_t)(t >> 1) & 1u) ^ 1u, 21);
+        const int st = t % NST, c0 = c_begin + t * 64;
+        mbar_wait(&y_empty[st], ((uint32_t)(t / NST) & 1u) ^ 1u, 21);
         uint8_t* y = sY + st * YST;
         mbar_expect_tx(&y_full[st], 2 * HALF_BYTES + (DKDV ? 512u : 0u));
         tma_load_2d(y, &mY0, &y_full[st], cy0, row0 + c0);
@@ -348,8 +401,8 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       constexpr uint32_t ID_T = idesc(128, 64, false, false), ID_ACC = idesc(128, 64, false, true);
       const uint32_t aX0 = smem_u32(sX0), aX1 = smem_u32(sX1), aE0 = smem_u32(sE0), aE1 = smem_u32(sE1);
       auto issue_t = [&](int t) {
-        const int st = t & 1;
-        mbar_wait(&y_full[st], (uint32_t)(t >> 1) & 1u, 22);
+        const int st = t % NST;
+        mbar_wait(&y_full[st], (uint32_t)(t / NST) & 1u, 22);
         tc_fence_after();
         const uint32_t aY0 = smem_u32(sY + st * YST), aY1 = aY0 + HALF_BYTES;
 #pragma unroll
@@ -366,7 +419,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
         mbar_wait(e_full, (uint32_t)t & 1u, 24);          // E_t is in shared memory and T_t has been consumed
         tc_fence_after();
         if (t + 1 < n_steps) issue_t(t + 1);
-        const int st = t & 1;
+        const int st = t % NST;
         const uint32_t aY0 = smem_u32(sY + st * YST), aY1 = aY0 + HALF_BYTES;
         const uint32_t acc = t > 0 ? 1u : 0u;
         if (DKDV) {
@@ -383,87 +436,114 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       umma_commit(acc_full);
     }
   } else {
+    // EW warpgroups of 4 warps: warp w owns TMEM lanes 32 (w % 4) .., warpgroup g = (w - 2) / 4 owns columns
+    // [g CW, (g + 1) CW) of T0 / T1 -- the backward has no row reductions, so the groups never talk.
+    // `lse` here is lse * log2(e) (written by the delta kernel); the 1/sqrt(dh) of dS is applied once, to
+    // the dK / dQ accumulators in the epilogue (exact: a power of two).
+    constexpr int CW = 64 / EW;
     const int r = (warp & 3) * 32 + lane;                 // stationary row inside the tile = TMEM lane
+    const int wg = (warp - 2) >> 2;
+    const int cw0 = wg * CW;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
-    const float c = rsqrtf((float)DH) * LOG2E, inv_sqrt = rsqrtf((float)DH);
+    const float c = rsqrtf((float)DH) * LOG2E;
     float my_lse2 = 0.f, my_delta = 0.f;
     if (!DKDV) {
-      my_lse2 = lse[((size_t)b * H + h) * T + x0 + r] * LOG2E;
+      my_lse2 = lse[((size_t)b * H + h) * T + x0 + r];
       my_delta = delta[((size_t)b * H + h) * T + x0 + r];
     }
     uint8_t* e0row = sE0 + r * 128;
     uint8_t* e1row = sE1 + r * 128;
+#ifdef PACI_ATTN_TIMING
+    long long tk[6] = {0, 0, 0, 0, 0, 0}, tprev = clock64(), tnow;
+#define TICK(i) do { tnow = clock64(); tk[i] += tnow - tprev; tprev = tnow; } while (0)
+#else
+#define TICK(i) do {} while (0)
+#endif
     for (int t = 0; t < n_steps; ++t) {
-      const int st = t & 1, c0 = c_begin + t * 64;
-      mbar_wait(t_full, (uint32_t)t & 1u, 25);
+      const int st = t % NST, c0 = c_begin + t * 64;
+      mbar_wait_many(t_full, (uint32_t)t & 1u, 25);
       tc_fence_after();
-      uint32_t s[64], dp[64];
-      tmem_ld32_nowait(tT0 + lane_off, s);
-      tmem_ld32_nowait(tT0 + lane_off + 32, s + 32);
-      tmem_ld32_nowait(tT1 + lane_off, dp);
-      tmem_ld32_nowait(tT1 + lane_off + 32, dp + 32);
+      TICK(0);
+      uint32_t s[CW], dp[CW];
+      tmem_ld_cols_nowait<CW>(tT0 + lane_off + cw0, s);
+      tmem_ld_cols_nowait<CW>(tT1 + lane_off + cw0, dp);
       tmem_ld_wait();
-      const float* st_lse = reinterpret_cast<const float*>(sStat + st * 512);
-      const float* st_del = st_lse + 64;
-      if (DKDV) mbar_wait(&y_full[st], (uint32_t)(t >> 1) & 1u, 26);   // the step's lse / delta have landed
-      // causal keep: query >= key.  DKDV: query = c0 + i, key = x0 + r.  DQ: query = x0 + r, key = c0 + i.
+      TICK(1);
+      const float4* pl = reinterpret_cast<const float4*>(sStat + st * 512) + cw0 / 4;   // lse2 of the step's 64 queries
+      const float4* pd = pl + 16;                                                        // delta
+      if (DKDV) mbar_wait_many(&y_full[st], (uint32_t)(t / NST) & 1u, 26);   // the step's lse / delta have landed
+      // causal keep: query >= key.  DKDV: query = c0 + col, key = x0 + r.  DQ: query = x0 + r, key = c0 + col.
+      // Only the two diagonal steps need the mask; `rel` is the diagonal's column inside this thread's slice.
       const bool diag = DKDV ? (c0 < x0 + 128) : (c0 + 63 > x0);
-      if (t > 0) mbar_wait(e_empty, (uint32_t)(t - 1) & 1u, 27);        // ACC_{t-1} has finished reading E
+      const int rel = x0 + r - c0 - cw0;
+      uint32_t wp[CW / 2], wd[CW / 2];
+      auto body = [&](auto masked) {
 #pragma unroll
-      for (int ch = 0; ch < 8; ++ch) {
-        uint32_t wp[4], wd[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          float pv[2], dv[2];
-#pragma unroll
-          for (int e = 0; e < 2; ++e) {
-            const int i = ch * 8 + 2 * u + e;
-            const float l2 = DKDV ? st_lse[i] * LOG2E : my_lse2;
-            const float dl = DKDV ? st_del[i] : my_delta;
-            float p = ex2(__uint_as_float(s[i]) * c - l2);
-            if (diag) {
-              const bool keep = DKDV ? (c0 + i >= x0 + r) : (x0 + r >= c0 + i);
-              p = keep ? p : 0.f;
-            }
-            pv[e] = p;
-            dv[e] = p * (__uint_as_float(dp[i]) - dl) * inv_sqrt;
+        for (int k4 = 0; k4 < CW / 4; ++k4) {
+          float l2[4] = {my_lse2, my_lse2, my_lse2, my_lse2}, dl[4] = {my_delta, my_delta, my_delta, my_delta};
+          if (DKDV) {
+            const float4 a4 = pl[k4], d4 = pd[k4];
+            l2[0] = a4.x; l2[1] = a4.y; l2[2] = a4.z; l2[3] = a4.w;
+            dl[0] = d4.x; dl[1] = d4.y; dl[2] = d4.z; dl[3] = d4.w;
           }
-          wp[u] = pack_bf16x2(pv[0], pv[1]);
-          wd[u] = pack_bf16x2(dv[0], dv[1]);
+          float pv[4], dv[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int i = 4 * k4 + e;
+            float pr = ex2(fmaf(__uint_as_float(s[i]), c, -l2[e]));
+            if (decltype(masked)::value) {
+              const bool keep = DKDV ? (i >= rel) : (i <= rel);
+              pr = keep ? pr : 0.f;
+            }
+            pv[e] = pr;
+            dv[e] = pr * (__uint_as_float(dp[i]) - dl[e]);
+          }
+          wp[2 * k4] = pack_bf16x2(pv[0], pv[1]); wp[2 * k4 + 1] = pack_bf16x2(pv[2], pv[3]);
+          wd[2 * k4] = pack_bf16x2(dv[0], dv[1]); wd[2 * k4 + 1] = pack_bf16x2(dv[2], dv[3]);
         }
-        const uint32_t off = (uint32_t)((ch ^ (r & 7)) << 4);
-        if (DKDV) sts128(e0row + off, wp[0], wp[1], wp[2], wp[3]);
-        sts128(e1row + off, wd[0], wd[1], wd[2], wd[3]);
+      };
+      if (diag) body(std::true_type{}); else body(std::false_type{});
+      TICK(2);
+      if (t > 0) mbar_wait_many(e_empty, (uint32_t)(t - 1) & 1u, 27);        // ACC_{t-1} has finished reading E
+      TICK(3);
+#pragma unroll
+      for (int ch = 0; ch < CW / 8; ++ch) {
+        const uint32_t off = (uint32_t)(((cw0 / 8 + ch) ^ (r & 7)) << 4);
+        if (DKDV) sts128(e0row + off, wp[4 * ch], wp[4 * ch + 1], wp[4 * ch + 2], wp[4 * ch + 3]);
+        sts128(e1row + off, wd[4 * ch], wd[4 * ch + 1], wd[4 * ch + 2], wd[4 * ch + 3]);
       }
       fence_async_smem();
       tc_fence_before();
       mbar_arrive(e_full);
+      TICK(4);
     }
-    // epilogue: accumulators -> bf16 rows of dqkv
-    mbar_wait(acc_full, 0, 28);
+#ifdef PACI_ATTN_TIMING
+    if (threadIdx.x == 64 && (blockIdx.x == 0 || blockIdx.x == 300 || blockIdx.x == 900))
+      printf("bwd dkdv=%d blk %d steps %d: wait_t %lld ldtm %lld compute %lld wait_e %lld sts+fence %lld (cycles per step)\n", (int)DKDV,
+             (int)blockIdx.x, n_steps, tk[0] / n_steps, tk[1] / n_steps, tk[2] / n_steps, tk[3] / n_steps, tk[4] / n_steps);
+#endif
+    // epilogue: accumulators -> bf16 rows of dqkv, 32-column chunks dealt round-robin to the warpgroups
+    mbar_wait_many(acc_full, 0, 28);
     tc_fence_after();
     bf16* orow = dqkv + ((size_t)row0 + x0 + r) * 3 * D + h * DH;
-    auto store_acc = [&](uint32_t taddr, bf16* dst) {
+    auto store_chunk = [&](uint32_t taddr, bf16* dst, float scale) {   // 32 fp32 columns -> 32 bf16
+      uint32_t ov[32];
+      tmem_ld32(taddr + lane_off, ov);
 #pragma unroll
-      for (int q = 0; q < 2; ++q) {
-        uint32_t ov[32];
-        tmem_ld32(taddr + lane_off + q * 32, ov);
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          uint4 w;
-          w.x = pack_bf16x2(__uint_as_float(ov[8 * i]), __uint_as_float(ov[8 * i + 1]));
-          w.y = pack_bf16x2(__uint_as_float(ov[8 * i + 2]), __uint_as_float(ov[8 * i + 3]));
-          w.z = pack_bf16x2(__uint_as_float(ov[8 * i + 4]), __uint_as_float(ov[8 * i + 5]));
-          w.w = pack_bf16x2(__uint_as_float(ov[8 * i + 6]), __uint_as_float(ov[8 * i + 7]));
-          *reinterpret_cast<uint4*>(dst + q * 32 + i * 8) = w;
-        }
+      for (int i = 0; i < 4; ++i) {
+        uint4 w;
+        w.x = pack_bf16x2(__uint_as_float(ov[8 * i]) * scale, __uint_as_float(ov[8 * i + 1]) * scale);
+        w.y = pack_bf16x2(__uint_as_float(ov[8 * i + 2]) * scale, __uint_as_float(ov[8 * i + 3]) * scale);
+        w.z = pack_bf16x2(__uint_as_float(ov[8 * i + 4]) * scale, __uint_as_float(ov[8 * i + 5]) * scale);
+        w.w = pack_bf16x2(__uint_as_float(ov[8 * i + 6]) * scale, __uint_as_float(ov[8 * i + 7]) * scale);
+        *reinterpret_cast<uint4*>(dst + i * 8) = w;
       }
     };
-    if (DKDV) {
-      store_acc(tA0, orow + 2 * D);   // dV
-      store_acc(tA1, orow + D);       // dK
-    } else {
-      store_acc(tA1, orow);           // dQ
+    const float inv_sqrt = rsqrtf((float)DH);
+    constexpr int N_CHUNKS = DKDV ? 4 : 2;                // DKDV: dV lo, dV hi, dK lo, dK hi.  DQ: dQ lo, dQ hi
+    for (int k = wg; k < N_CHUNKS; k += EW) {             // warp-uniform
+      if (DKDV) store_chunk((k < 2 ? tA0 : tA1) + (k & 1) * 32, orow + (k < 2 ? 2 * D : D) + (k & 1) * 32, k < 2 ? 1.f : inv_sqrt);
+      else store_chunk(tA1 + k * 32, orow + k * 32, inv_sqrt);
     }
   }
   tc_fence_before();
@@ -477,7 +557,8 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
 
 // delta[b,h,t] = sum_d dO[b,t,h,d] * O[b,t,h,d]: 8 threads per (b,t,h), one 16-byte vector each
 __global__ void __launch_bounds__(256) attn_delta_tc_kernel(size_t n_vec, int T, int H, const bf16* __restrict__ dout,
-                                                            const bf16* __restrict__ o, float* __restrict__ delta) {
+                                                            const bf16* __restrict__ o, const float* __restrict__ lse,
+                                                            float* __restrict__ delta, float* __restrict__ lse2) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   float acc = 0.f;
   if (i < n_vec) {
@@ -492,13 +573,15 @@ __global__ void __launch_bounds__(256) attn_delta_tc_kernel(size_t n_vec, int T,
   if (i < n_vec && (threadIdx.x & 7) == 0) {
     const size_t hv = i >> 3;                  // (b*T + t)*H + h
     const size_t bt = hv / H;
-    delta[((bt / T) * H + hv % H) * T + bt % T] = acc;
+    const size_t idx = ((bt / T) * H + hv % H) * T + bt % T;
+    delta[idx] = acc;
+    lse2[idx] = lse[idx] * LOG2E;                         // the backward kernels work in the exp2 domain
   }
 }
 
 }  // namespace
 
-size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H) { return (size_t)mu * H * T * sizeof(float); }
+size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H) { return 2 * (size_t)mu * H * T * sizeof(float); }
 
 int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
                      void* dqkv, float* scratch, cudaStream_t s) {
@@ -512,20 +595,21 @@ int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, co
   if ((rc = make_tensor_map(&d64, dout, (uint64_t)D, rows, (uint64_t)D, 64, 64, 2))) return rc;
   static bool attr_set = false;
   if (!attr_set) {
-    PACI_CUDA_OK(cudaFuncSetAttribute(attn_bwd_tc_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BWD_SMEM));
-    PACI_CUDA_OK(cudaFuncSetAttribute(attn_bwd_tc_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)BWD_SMEM));
+    PACI_CUDA_OK(cudaFuncSetAttribute(attn_bwd_tc_kernel<true, BWD_EW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bwd_smem(true)));
+    PACI_CUDA_OK(cudaFuncSetAttribute(attn_bwd_tc_kernel<false, BWD_EW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bwd_smem(false)));
     attr_set = true;
   }
   float* delta = scratch;
+  float* lse2 = scratch + (size_t)mu * H * T;
   const size_t n_vec = (size_t)mu * T * D / 8;
   PACI_LAUNCH(attn_delta_tc_kernel, ceil_div((long long)n_vec, 256), 256, 0, s, n_vec, T, H, (const bf16*)dout,
-              (const bf16*)o, delta);
+              (const bf16*)o, lse, delta, lse2);
   const int grid = (T / 128) * H * mu;
   // dK, dV: stationary K_j, V_j (qkv, 128-row boxes); streamed Q_i (qkv), dO_i (dout), 64-row boxes
-  PACI_LAUNCH(attn_bwd_tc_kernel<true>, grid, BWD_THREADS, BWD_SMEM, s, q128, q128, q64, d64, T, H, lse, delta,
+  PACI_LAUNCH((attn_bwd_tc_kernel<true, BWD_EW>), grid, BWD_THREADS, bwd_smem(true), s, q128, q128, q64, d64, T, H, lse2, delta,
               (bf16*)dqkv);
   // dQ: stationary Q_i (qkv), dO_i (dout); streamed K_j, V_j (qkv)
-  PACI_LAUNCH(attn_bwd_tc_kernel<false>, grid, BWD_THREADS, BWD_SMEM, s, q128, d128, q64, q64, T, H, lse, delta,
+  PACI_LAUNCH((attn_bwd_tc_kernel<false, BWD_EW>), grid, BWD_THREADS, bwd_smem(false), s, q128, d128, q64, q64, T, H, lse2, delta,
               (bf16*)dqkv);
   return PACI_OK;
 }

@@ -1,5 +1,6 @@
 // ops.cu -- backend dispatch (fp32 -> FFMA kernels, bf16 -> tcgen05 / tensor-core kernels) and the
 // op-level C-ABI entry points used by the kernel parity tests and the per-kernel roofline benches.
+#include <algorithm>
 #include <cstdlib>
 #include <cstring>
 
@@ -45,6 +46,7 @@ int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, co
 int attention_bwd_mma(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
                       void* dqkv, float* scratch, cudaStream_t s);
 size_t attention_bwd_mma_scratch_bytes(int mu, int T, int H);
+size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H);
 
 // algorithmic work: causal half of QK^T and PV (2 * mu*H*T*T*dh flops forward, twice that backward)
 int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse, cudaStream_t s) {
@@ -72,7 +74,8 @@ int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, con
 
 size_t attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh) {
   size_t simt = (size_t)mu * H * T * sizeof(float);
-  if (dtype == PACI_BF16 && dh == 64) return std::max(simt, attention_bwd_mma_scratch_bytes(mu, T, H));
+  if (dtype == PACI_BF16 && dh == 64)
+    return std::max({simt, attention_bwd_mma_scratch_bytes(mu, T, H), attention_bwd_tc_scratch_bytes(mu, T, H)});
   return simt;
 }
 

@@ -1,0 +1,125 @@
+"""-m gpu: parity at BASELINE.json's full sizes (cfg 3, GPT-2 Medium: D 1024, H 16, T 1024, micro-batch 8,
+V 50257), in the launch configuration bench.py times, on SAMPLED outputs the oracle can compute one by one
+(a full fp64 pass over 8192 tokens is 18 TFLOP), plus whole-stage parity at full width with micro-batch 1
+("the oracle is used for bf16 parity at full width but mu = 1").  bf16 gates: rel-L2 <= 2e-2."""
+import numpy as np
+import pytest
+import torch
+
+import synth
+from oracle import model
+from paper_2606_07881_b200 import binding as pb
+from gpu_util import TOL, host, rel_l2, rounded
+import gpu_util
+
+pytestmark = pytest.mark.gpu
+lib = pb.lib
+D, H, T, MU, V = 1024, 16, 1024, 8, 50257
+M = MU * T
+VPAD = (V + 63) // 64 * 64
+
+
+def ck(rc):
+    assert rc == 0, lib.paci_last_error().decode()
+
+
+def S0():
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _bf(a):
+    return gpu_util.dev(a, pb.BF16)
+
+
+@pytest.mark.parametrize("layout,Mg,Ng,Kg,accum", [(0, M, 4 * D, D, 0), (0, M, D, 4 * D, 0), (1, M, D, 3 * D, 0),
+                                                    (2, 4 * D, D, M, 1), (2, D, D, M, 1)])
+def test_gemm_full_size_sampled_rows(layout, Mg, Ng, Kg, accum):
+    """The tcgen05 GEMM at the shapes of one cfg-3 block (MLP-up / MLP-down forward, QKV dgrad, W1 and Wo wgrad
+    with split-K and the beta = 1 TMA reduce-add epilogue): 24 sampled output rows against fp64 dot products."""
+    rng = np.random.default_rng(layout * 7 + Ng)
+    g = torch.Generator(device="cuda").manual_seed(layout * 13 + Kg)
+    a_shape = (Mg, Kg) if layout != 2 else (Kg, Mg)
+    b_shape = (Ng, Kg) if layout == 0 else (Kg, Ng)
+    A = (torch.randn(a_shape, device="cuda", generator=g) * 0.5).to(torch.bfloat16)
+    B = (torch.randn(b_shape, device="cuda", generator=g) * 0.5).to(torch.bfloat16)
+    bias = torch.randn(Ng, device="cuda", generator=g) if not accum else None
+    C = torch.full((Mg, Ng), 2.0, device="cuda") if accum else torch.empty(Mg, Ng, device="cuda", dtype=torch.bfloat16)
+    ck(lib.paci_op_gemm(pb.BF16, layout, Mg, Ng, Kg, A.data_ptr(), a_shape[1], B.data_ptr(), b_shape[1],
+                        bias.data_ptr() if bias is not None else None, C.data_ptr(), Ng, accum, S0()))
+    torch.cuda.synchronize()
+    rows = np.unique(np.concatenate([rng.integers(0, Mg, 20), [0, 127, 128, Mg - 1]]))
+    Ah, Bh = host(A), host(B)
+    Bm = Bh.T if layout == 0 else Bh                                   # [K, N]
+    for r in rows:
+        a_row = Ah[r] if layout != 2 else Ah[:, r]
+        ref = a_row @ Bm + (host(bias) if bias is not None else 2.0)
+        assert rel_l2(host(C[r]), ref) < (5e-3 if not accum else 1e-4), (layout, int(r))
+
+
+def test_attention_full_size_sampled_heads():
+    """tcgen05 attention forward / backward at mu 8, T 1024, H 16: three sampled (batch, head) pairs against the
+    oracle run on that head alone (the heads are independent); lse as well."""
+    rng = np.random.default_rng(5)
+    qkv = rng.standard_normal((MU, T, 3 * D)) * 0.7
+    do = rng.standard_normal((MU, T, D)) * 0.1
+    qd, dod = _bf(qkv), _bf(do)
+    o = torch.empty(MU, T, D, device="cuda", dtype=torch.bfloat16)
+    lse = torch.empty(MU, H, T, device="cuda")
+    ck(lib.paci_op_attention_fwd(pb.BF16, MU, T, H, 64, qd.data_ptr(), o.data_ptr(), lse.data_ptr(), S0()))
+    nb = lib.paci_op_attention_bwd_scratch_bytes(pb.BF16, MU, T, H, 64)
+    scratch = torch.empty(nb, device="cuda", dtype=torch.uint8)
+    dqkv = torch.empty_like(qd)
+    ck(lib.paci_op_attention_bwd(pb.BF16, MU, T, H, 64, dod.data_ptr(), qd.data_ptr(), o.data_ptr(), lse.data_ptr(),
+                                 dqkv.data_ptr(), scratch.data_ptr(), S0()))
+    torch.cuda.synchronize()
+    qh, doh, oh, dqh, lh = host(qd), host(dod), host(o), host(dqkv), host(lse)
+    for b, h in [(0, 0), (3, 7), (7, 15)]:
+        sl = slice(h * 64, (h + 1) * 64)
+        one = np.concatenate([qh[b:b + 1, :, sl], qh[b:b + 1, :, D + h * 64:D + (h + 1) * 64],
+                              qh[b:b + 1, :, 2 * D + h * 64:2 * D + (h + 1) * 64]], axis=-1)      # [1, T, 192]
+        o_ref, stash = model.attention_fwd(one, 1)
+        assert rel_l2(oh[b, :, sl], o_ref[0]) < TOL[pb.BF16] / 4, (b, h)
+        q, k = stash[0], stash[1]
+        s = np.where(np.tril(np.ones((T, T), bool)), q[0, 0] @ k[0, 0].T / 8.0, -np.inf)
+        lse_ref = np.log(np.exp(s - s.max(-1, keepdims=True)).sum(-1)) + s.max(-1)
+        assert rel_l2(lh[b, h], lse_ref) < 1e-3
+        d_ref = model.attention_bwd(doh[b:b + 1, :, sl], stash)[0]                                 # [T, 192]
+        got = np.concatenate([dqh[b, :, sl], dqh[b, :, D + h * 64:D + (h + 1) * 64],
+                              dqh[b, :, 2 * D + h * 64:2 * D + (h + 1) * 64]], axis=-1)
+        assert rel_l2(got, d_ref) < TOL[pb.BF16] / 2, (b, h)
+
+
+@pytest.mark.parametrize("s,S,L", [(1, 4, 1), (3, 4, 0)])
+def test_stage_full_width_micro_batch_1(s, S, L):
+    """One interior block and the head stage (final LN, LM head over V = 50257, cross-entropy) at full width,
+    micro-batch 1, through paci_forward / paci_backward: loss, boundary gradients and every accumulated
+    parameter gradient against the oracle."""
+    mu = 1
+    spec = model.StageSpec(s, S, L, D, H, T, mu, V)
+    params = synth.stage_params(3, s, S, L, D, V, T, perturbed=True)
+    st = pb.Stage(pb.make_config(s, S, L, D, H, T, mu, 1, V, pb.BF16))
+    st.load_params(params)
+    rng = np.random.default_rng(17)
+    tok = synth.tokens(17, 1, mu, T, V, "zipf")[0]
+    tgt = tok[:, 1:].copy()
+    h = rounded(rng.standard_normal((mu, T, D)), pb.BF16)
+    dout = rounded(rng.standard_normal((mu, T, D)) * 0.1, pb.BF16)
+    P = {n: np.asarray(a, np.float64) for n, a in params.items()}
+    ref_out, stash = model.stage_forward(spec, P, h, tgt.astype(np.int64))
+    ref_din, ref_g = model.stage_backward(spec, P, stash, None if spec.has_head else dout)
+    hd = _bf(h)
+    tg = torch.from_numpy(tgt).cuda() if spec.has_head else None
+    out = torch.zeros(1, device="cuda") if spec.has_head else torch.empty(mu, T, D, device="cuda", dtype=torch.bfloat16)
+    din = torch.empty(mu, T, D, device="cuda", dtype=torch.bfloat16)
+    st.forward(0, hd, tg, out)
+    st.backward(0, None if spec.has_head else _bf(dout), din)
+    torch.cuda.synchronize()
+    if spec.has_head:
+        assert abs(out.item() - ref_out) / abs(ref_out) < 5e-3
+    else:
+        assert rel_l2(host(out), ref_out) < TOL[pb.BF16]
+    assert rel_l2(host(din), ref_din) < TOL[pb.BF16]
+    for name, g in ref_g.items():
+        got = st.read(name, pb.GRAD_ACCUM)
+        assert rel_l2(got, g) < TOL[pb.BF16], (name, rel_l2(got, g))
+    st.close()

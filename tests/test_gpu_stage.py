@@ -56,6 +56,7 @@ CASES = [  # dtype, s, S, L, D, H, T, mu, V
     (pb.BF16, 1, 2, 1, 128, 2, 64, 2, 1000),   # ragged vocab (1000 -> padded 1024)
     (pb.BF16, 1, 3, 2, 256, 4, 192, 2, 512),   # interior, several tiles + ragged M tail (384 rows)
     (pb.BF16, 0, 1, 1, 128, 2, 128, 1, 777),   # tied head
+    (pb.BF16, 1, 3, 1, 256, 4, 384, 1, 512),   # T % 128 == 0: tcgen05 attention over several key blocks
 ]
 
 
