@@ -74,6 +74,20 @@ template <> __device__ __forceinline__ void store_vec<bf16>(bf16* p, const float
   for (int i = 0; i < 4; ++i) h[i] = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]);
   *reinterpret_cast<uint4*>(p) = t;
 }
+// raw 16-byte vector kept PACKED in registers (4 registers instead of Vec<T>::N) and unpacked on use
+template <typename T> __device__ __forceinline__ uint4 load_raw(const T* p) { return *reinterpret_cast<const uint4*>(p); }
+template <typename T> __device__ __forceinline__ void unpack_raw(const uint4& t, float (&v)[Vec<T>::N]);
+template <> __device__ __forceinline__ void unpack_raw<float>(const uint4& t, float (&v)[4]) {
+  v[0] = __uint_as_float(t.x); v[1] = __uint_as_float(t.y); v[2] = __uint_as_float(t.z); v[3] = __uint_as_float(t.w);
+}
+template <> __device__ __forceinline__ void unpack_raw<bf16>(const uint4& t, float (&v)[8]) {
+  const uint32_t w[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {                 // bf16 -> fp32 is a 16-bit shift
+    v[2 * i] = __uint_as_float(w[i] << 16);
+    v[2 * i + 1] = __uint_as_float(w[i] & 0xffff0000u);
+  }
+}
 // N consecutive fp32 values (N = 4 or 8) as float4 loads
 template <int N> __device__ __forceinline__ void load_f32(const float* p, float (&v)[N]) {
 #pragma unroll

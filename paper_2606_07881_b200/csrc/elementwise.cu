@@ -148,41 +148,44 @@ int ln_fwd(int dtype, int rows, int D, const void* x, const void* res, const flo
 // (A single kernel holding the 3 x D/32 column partials per lane needed > 200 registers: one 8-warp CTA per
 // SM and 0.13 of HBM peak.)
 template <typename T, int NV>
-__global__ void __launch_bounds__(256) ln_bwd_dx_kernel(int rows, int D, const T* __restrict__ dy,
-                                                        const T* __restrict__ x, const float* __restrict__ mean,
-                                                        const float* __restrict__ rstd,
-                                                        const float* __restrict__ g, const T* __restrict__ dres,
-                                                        T* __restrict__ dx) {
+__global__ void __launch_bounds__(256, 3) ln_bwd_dx_kernel(int rows, int D, const T* __restrict__ dy,
+                                                           const T* __restrict__ x, const float* __restrict__ mean,
+                                                           const float* __restrict__ rstd,
+                                                           const float* __restrict__ g, const T* __restrict__ dres,
+                                                           T* __restrict__ dx) {
   constexpr int V = Vec<T>::N;
   const int lane = threadIdx.x & 31;
   const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (row >= rows) return;
   const int nvec = D / V;
   const size_t base = (size_t)row * D;
-  const float mu = mean[row], rs = rstd[row];
-  float dyv[NV][V], xh[NV][V], rv[NV][V];
+  // the row stays PACKED in registers (3 x NV x 4 registers) and is unpacked once per pass, which leaves
+  // room for three 8-warp CTAs per SM: more rows, i.e. more bytes, in flight
+  uint4 rdy[NV], rx[NV], rr[NV];
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
     const int c = lane + 32 * i;
     if (c < nvec) {
-      load_vec<T>(dy + base + (size_t)c * V, dyv[i]);
-      load_vec<T>(x + base + (size_t)c * V, xh[i]);
-      if (dres != nullptr) load_vec<T>(dres + base + (size_t)c * V, rv[i]);
+      rdy[i] = load_raw<T>(dy + base + (size_t)c * V);
+      rx[i] = load_raw<T>(x + base + (size_t)c * V);
+      if (dres != nullptr) rr[i] = load_raw<T>(dres + base + (size_t)c * V);
     }
   }
+  const float mu = mean[row], rs = rstd[row];
   float s1 = 0.f, s2 = 0.f;
 #pragma unroll
   for (int i = 0; i < NV; ++i) {
     const int c = lane + 32 * i;
     if (c < nvec) {
-      float gg[V];
+      float gg[V], dyv[V], xv[V];
       load_f32<V>(g + (size_t)c * V, gg);
+      unpack_raw<T>(rdy[i], dyv);
+      unpack_raw<T>(rx[i], xv);
 #pragma unroll
       for (int j = 0; j < V; ++j) {
-        xh[i][j] = (xh[i][j] - mu) * rs;
-        dyv[i][j] *= gg[j];
-        s1 += dyv[i][j];
-        s2 += dyv[i][j] * xh[i][j];
+        const float gd = dyv[j] * gg[j];
+        s1 += gd;
+        s2 += gd * ((xv[j] - mu) * rs);
       }
     }
   }
@@ -193,20 +196,26 @@ __global__ void __launch_bounds__(256) ln_bwd_dx_kernel(int rows, int D, const T
   for (int i = 0; i < NV; ++i) {
     const int c = lane + 32 * i;
     if (c < nvec) {
-      float o[V];
+      float gg[V], dyv[V], xv[V], o[V];
+      load_f32<V>(g + (size_t)c * V, gg);
+      unpack_raw<T>(rdy[i], dyv);
+      unpack_raw<T>(rx[i], xv);
 #pragma unroll
-      for (int j = 0; j < V; ++j) {
-        o[j] = rs * (dyv[i][j] - s1 - xh[i][j] * s2);
-        if (dres != nullptr) o[j] += rv[i][j];
+      for (int j = 0; j < V; ++j) o[j] = rs * (dyv[j] * gg[j] - s1 - ((xv[j] - mu) * rs) * s2);
+      if (dres != nullptr) {
+        float r[V];
+        unpack_raw<T>(rr[i], r);
+#pragma unroll
+        for (int j = 0; j < V; ++j) o[j] += r[j];
       }
       store_vec<T>(dx + base + (size_t)c * V, o);
     }
   }
 }
 
-constexpr int LNC_TX = 128, LNC_TY = 4, LNC_U = 4;
+constexpr int LNC_TX = 128, LNC_TY = 2, LNC_U = 4;
 template <typename T>
-__global__ void __launch_bounds__(LNC_TX * LNC_TY) ln_bwd_cols_kernel(int rows, int D, const T* __restrict__ dy,
+__global__ void __launch_bounds__(LNC_TX * LNC_TY, 3) ln_bwd_cols_kernel(int rows, int D, const T* __restrict__ dy,
                                                                        const T* __restrict__ x,
                                                                        const float* __restrict__ mean,
                                                                        const float* __restrict__ rstd,
@@ -225,15 +234,16 @@ __global__ void __launch_bounds__(LNC_TX * LNC_TY) ln_bwd_cols_kernel(int rows, 
   const int stride = gridDim.y * LNC_TY;
   if (live) {
     for (int r0 = blockIdx.y * LNC_TY + ty; r0 < rows; r0 += LNC_U * stride) {
-      float dyv[LNC_U][V], xv[LNC_U][V], dxv[LNC_U][V], mu[LNC_U], rs[LNC_U];
+      uint4 rdy[LNC_U], rx[LNC_U], rdx[LNC_U];
+      float mu[LNC_U], rs[LNC_U];
 #pragma unroll
       for (int u = 0; u < LNC_U; ++u) {
         const int r = r0 + u * stride;
         if (r < rows) {
           const size_t off = (size_t)r * D + c;
-          load_vec<T>(dy + off, dyv[u]);
-          load_vec<T>(x + off, xv[u]);
-          if (Gcol != nullptr) load_vec<T>(dx + off, dxv[u]);
+          rdy[u] = load_raw<T>(dy + off);
+          rx[u] = load_raw<T>(x + off);
+          if (Gcol != nullptr) rdx[u] = load_raw<T>(dx + off);
           mu[u] = __ldg(mean + r);
           rs[u] = __ldg(rstd + r);
         }
@@ -241,11 +251,19 @@ __global__ void __launch_bounds__(LNC_TX * LNC_TY) ln_bwd_cols_kernel(int rows, 
 #pragma unroll
       for (int u = 0; u < LNC_U; ++u) {
         if (r0 + u * stride < rows) {
+          float dyv[V], xv[V];
+          unpack_raw<T>(rdy[u], dyv);
+          unpack_raw<T>(rx[u], xv);
 #pragma unroll
           for (int j = 0; j < V; ++j) {
-            ag[j] += dyv[u][j] * ((xv[u][j] - mu[u]) * rs[u]);
-            ab[j] += dyv[u][j];
-            if (Gcol != nullptr) ac[j] += dxv[u][j];
+            ag[j] += dyv[j] * ((xv[j] - mu[u]) * rs[u]);
+            ab[j] += dyv[j];
+          }
+          if (Gcol != nullptr) {
+            float dxv[V];
+            unpack_raw<T>(rdx[u], dxv);
+#pragma unroll
+            for (int j = 0; j < V; ++j) ac[j] += dxv[j];
           }
         }
       }
@@ -288,7 +306,7 @@ static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float*
   }
 #undef LNB_CASE
   const int gx = ceil_div(D / V, LNC_TX);
-  int gy = std::max(1, num_sms() / gx);
+  int gy = std::max(1, 3 * num_sms() / gx);
   gy = std::min(gy, ceil_div(rows, LNC_TY));
   PACI_LAUNCH((ln_bwd_cols_kernel<T>), dim3(gx, gy), dim3(LNC_TX, LNC_TY), 0, s, rows, D, (const T*)dy,
               (const T*)x, mean, rstd, (const T*)dx, Gg, Gb, Gcol);
