@@ -363,6 +363,61 @@ def run_ours(args, c, name):
     return 0
 
 
+
+# ------------------------------------------------------------------------------------ k sweep (configs[3])
+def run_k_sweep(args, c, name):
+    """BASELINE.json configs[3]: the same model split into S emulated stages, k in {1,2,4,8}: PACI and
+    1F1B-flush (groups of m_f = k micro-batches, Table 4's matched comparison) on the same GPU.
+    Per k: crossed-update counts Delta_{m,s} (max per stage against the bound ceil((S-1-s)/k), Eq. 10
+    P:398), versions, device time of the run, and the EMULATED pipeline step time: one GPU serialises the
+    stages, so bubbles cannot show in wall time; the virtual makespan is the schedule's logical slot count
+    (every stage does at most one F or B per slot, `n_slots` of paci_pipeline_run) x the measured mean
+    op time (t_F + t_B) / 2 of an interior stage.  flush / PACI is then compared with Eq. 3."""
+    import math
+    import torch
+    from paper_2606_07881_b200 import binding as pb
+    import synth
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    S, mu, T, n = c["S"], c["mu"], c["T"], c["n_micro"]
+    tok = torch.from_numpy(synth.tokens(SEED, n, mu, T, c["V"], c["dist"])).cuda()
+    rows = []
+    for k in (1, 2, 4, 8):
+        ck = dict(c, k=k)
+        row = {"k": k, "bound_max": math.ceil((S - 1) / k)}
+        for mode, tag in ((pb.MODE_PACI, "paci"), (pb.MODE_FLUSH, "flush")):
+            stages, pipe = build_pipeline(pb, ck, "cuda:0")
+            pipe.run(tok, ck["lr"], mode=mode, want_delta=False)              # warm-up run
+            out = pipe.run(tok, ck["lr"], mode=mode)
+            d = out["delta"]
+            row[tag] = {"ms": out["elapsed_ms"], "n_slots": int(out["n_slots"]),
+                        "max_delta_per_stage": [int(x) for x in d.max(axis=1)],
+                        "versions": [int(v) for v in out["version"]],
+                        "tokens_per_s_per_stage_step": S * n * mu * T / (out["elapsed_ms"] * 1e-3)}
+            if tag == "paci":
+                row["bound_per_stage"] = [math.ceil((S - 1 - s) / k) for s in range(S)]
+                row["bound_holds"] = all(a <= b for a, b in zip(row[tag]["max_delta_per_stage"], row["bound_per_stage"]))
+                st = per_stage_times(pb, torch, ck, stages, reps=2)[1]          # an interior stage
+                row["t_op_ms"] = (st["t_fwd_ms"] + st["t_bwd_ms"]) / 2
+            pipe.close()
+            for s_ in stages:
+                s_.close()
+            del stages, pipe
+            torch.cuda.empty_cache()
+        t_op = row["t_op_ms"]
+        row["virtual_ms"] = {"paci": row["paci"]["n_slots"] * t_op, "flush": row["flush"]["n_slots"] * t_op}
+        # steady state: PACI needs 2k slots per k micro-batches, a flush group (k + S - 1) * 2
+        row["eta_flush_eq3"] = k / (k + S - 1)
+        row["eta_measured_slots"] = 2 * n / row["flush"]["n_slots"] if row["flush"]["n_slots"] else None   # PACI steady state: 2 slots per micro-batch
+        rows.append(row)
+    line = {"metric": "k sweep: crossed updates and emulated step time, PACI vs 1F1B-flush", "n_gpus": 1,
+            "config": {"workload": workload_name(name, c), "n_microbatches": n}, "data": "synthetic",
+            "dtype": c["dtype"], "sweep": rows}
+    print(json.dumps(line))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -374,10 +429,13 @@ def main():
                     help="time every n-th library op with CUDA events; a sampled op runs alone on the GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stage-times", action="store_true")
+    ap.add_argument("--k-sweep", action="store_true", help="BASELINE.json configs[3]: k in {1,2,4,8}, PACI vs flush")
     args = ap.parse_args()
     c = CONFIGS[args.config]
     if args.impl == "reference":
         return run_reference(args, c, args.config)
+    if args.k_sweep:
+        return run_k_sweep(args, CONFIGS["medium8"] if args.config == "medium" else c, "medium8" if args.config == "medium" else args.config)
     return run_ours(args, c, args.config)
 
 
