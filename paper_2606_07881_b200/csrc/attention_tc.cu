@@ -325,7 +325,8 @@ template <bool DKDV, int EW>
 __global__ void __launch_bounds__(64 + 128 * EW, 2)
 attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constant__ CUtensorMap mX1,
                    const __grid_constant__ CUtensorMap mY0, const __grid_constant__ CUtensorMap mY1, int T, int H,
-                   const float* __restrict__ lse, const float* __restrict__ delta, bf16* __restrict__ dqkv) {
+                   const float* __restrict__ lse, const float* __restrict__ delta, bf16* __restrict__ dqkv,
+                   float* __restrict__ Gbias) {
   extern __shared__ __align__(1024) uint8_t smem[];
   constexpr uint32_t YST = 2 * HALF_BYTES;               // one ring stage: Y0, Y1 (1024-byte aligned tiles)
   uint8_t* sX0 = smem;
@@ -526,7 +527,10 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
     mbar_wait_many(acc_full, 0, 28);
     tc_fence_after();
     bf16* orow = dqkv + ((size_t)row0 + x0 + r) * 3 * D + h * DH;
-    auto store_chunk = [&](uint32_t taddr, bf16* dst, float scale) {   // 32 fp32 columns -> 32 bf16
+    // Gbias (fp32 [3D], may be NULL): the bias gradient of the QKV projection = column sums of dqkv over all
+    // tokens (row a15), taken here from the ROUNDED values being stored: one warp-shuffle reduction over the
+    // warp's 32 rows per column, then one atomic per column per warp -- no separate pass over dqkv.
+    auto store_chunk = [&](uint32_t taddr, bf16* dst, float scale, float* gcol) {   // 32 fp32 columns -> 32 bf16
       uint32_t ov[32];
       tmem_ld32(taddr + lane_off, ov);
 #pragma unroll
@@ -537,13 +541,30 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
         w.z = pack_bf16x2(__uint_as_float(ov[8 * i + 4]) * scale, __uint_as_float(ov[8 * i + 5]) * scale);
         w.w = pack_bf16x2(__uint_as_float(ov[8 * i + 6]) * scale, __uint_as_float(ov[8 * i + 7]) * scale);
         *reinterpret_cast<uint4*>(dst + i * 8) = w;
+        if (gcol != nullptr) {
+          const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const float lo = warp_sum(__uint_as_float(ww[u] << 16));
+            const float hi = warp_sum(__uint_as_float(ww[u] & 0xffff0000u));
+            if (lane == 0) {
+              atomicAdd(gcol + 8 * i + 2 * u, lo);
+              atomicAdd(gcol + 8 * i + 2 * u + 1, hi);
+            }
+          }
+        }
       }
     };
     const float inv_sqrt = rsqrtf((float)DH);
     constexpr int N_CHUNKS = DKDV ? 4 : 2;                // DKDV: dV lo, dV hi, dK lo, dK hi.  DQ: dQ lo, dQ hi
     for (int k = wg; k < N_CHUNKS; k += EW) {             // warp-uniform
-      if (DKDV) store_chunk((k < 2 ? tA0 : tA1) + (k & 1) * 32, orow + (k < 2 ? 2 * D : D) + (k & 1) * 32, k < 2 ? 1.f : inv_sqrt);
-      else store_chunk(tA1 + k * 32, orow + k * 32, inv_sqrt);
+      if (DKDV) {
+        const int col = (k < 2 ? 2 * D : D) + (k & 1) * 32;
+        store_chunk((k < 2 ? tA0 : tA1) + (k & 1) * 32, orow + col, k < 2 ? 1.f : inv_sqrt,
+                    Gbias != nullptr ? Gbias + h * DH + col : nullptr);
+      } else {
+        store_chunk(tA1 + k * 32, orow + k * 32, inv_sqrt, Gbias != nullptr ? Gbias + h * DH + k * 32 : nullptr);
+      }
     }
   }
   tc_fence_before();
@@ -584,7 +605,7 @@ __global__ void __launch_bounds__(256) attn_delta_tc_kernel(size_t n_vec, int T,
 size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H) { return 2 * (size_t)mu * H * T * sizeof(float); }
 
 int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
-                     void* dqkv, float* scratch, cudaStream_t s) {
+                     void* dqkv, float* scratch, float* Gbias, cudaStream_t s) {
   const int D = H * DH;
   const uint64_t rows = (uint64_t)mu * T;
   CUtensorMap q128, q64, d128, d64;
@@ -607,10 +628,10 @@ int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, co
   const int grid = (T / 128) * H * mu;
   // dK, dV: stationary K_j, V_j (qkv, 128-row boxes); streamed Q_i (qkv), dO_i (dout), 64-row boxes
   PACI_LAUNCH((attn_bwd_tc_kernel<true, BWD_EW>), grid, BWD_THREADS, bwd_smem(true), s, q128, q128, q64, d64, T, H, lse2, delta,
-              (bf16*)dqkv);
+              (bf16*)dqkv, Gbias);
   // dQ: stationary Q_i (qkv), dO_i (dout); streamed K_j, V_j (qkv)
   PACI_LAUNCH((attn_bwd_tc_kernel<false, BWD_EW>), grid, BWD_THREADS, bwd_smem(false), s, q128, d128, q64, q64, T, H, lse2, delta,
-              (bf16*)dqkv);
+              (bf16*)dqkv, Gbias);
   return PACI_OK;
 }
 

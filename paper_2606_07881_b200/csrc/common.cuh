@@ -161,7 +161,7 @@ int add_vec(int dtype, size_t n, const void* a, const void* b, void* out, cudaSt
 int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,
                   cudaStream_t s);
 int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv, const void* o,
-                  const float* lse, void* dqkv, float* scratch, cudaStream_t s);
+                  const float* lse, void* dqkv, float* scratch, float* Gbias, cudaStream_t s);
 size_t attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh);
 int attention_fwd_simt(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,
                        cudaStream_t s);

@@ -42,7 +42,7 @@ int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, con
 int attention_fwd_mma(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
 int attention_fwd_tc(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
 int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
-                     void* dqkv, float* scratch, cudaStream_t s);
+                     void* dqkv, float* scratch, float* Gbias, cudaStream_t s);
 int attention_bwd_mma(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
                       void* dqkv, float* scratch, cudaStream_t s);
 size_t attention_bwd_mma_scratch_bytes(int mu, int T, int H);
@@ -60,16 +60,25 @@ int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void
   return attention_fwd_simt(dtype, mu, T, H, dh, qkv, o, lse, s);
 }
 
+// Gbias (fp32 [3 H dh], may be NULL) += column sums of dqkv: the QKV bias gradient (row a15).  The tcgen05
+// kernels take it in their epilogue; the other backends run the column-sum kernel over dqkv afterwards.
 int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv, const void* o,
-                  const float* lse, void* dqkv, float* scratch, cudaStream_t s) {
-  const double e = dtype == PACI_BF16 ? 2.0 : 4.0, nd = (double)mu * T * H * dh;
-  ProfScope prof(PC_ATTN_BWD, 4.0 * mu * H * (double)T * T * dh, e * 8.0 * nd + 4.0 * mu * H * T, s);
-  if (dtype == PACI_BF16 && attn_backend_tensor()) {
-    if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
-    if (T % 128 == 0 && attn_backend_tcgen05()) return attention_bwd_tc(mu, T, H, dout, qkv, o, lse, dqkv, scratch, s);
-    return attention_bwd_mma(mu, T, H, dout, qkv, o, lse, dqkv, scratch, s);
+                  const float* lse, void* dqkv, float* scratch, float* Gbias, cudaStream_t s) {
+  int rc;
+  {
+    const double e = dtype == PACI_BF16 ? 2.0 : 4.0, nd = (double)mu * T * H * dh;
+    ProfScope prof(PC_ATTN_BWD, 4.0 * mu * H * (double)T * T * dh, e * 8.0 * nd + 4.0 * mu * H * T, s);
+    if (dtype == PACI_BF16 && attn_backend_tensor()) {
+      if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
+      if (T % 128 == 0 && attn_backend_tcgen05())
+        return attention_bwd_tc(mu, T, H, dout, qkv, o, lse, dqkv, scratch, Gbias, s);
+      rc = attention_bwd_mma(mu, T, H, dout, qkv, o, lse, dqkv, scratch, s);
+    } else {
+      rc = attention_bwd_simt(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, s);
+    }
   }
-  return attention_bwd_simt(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, s);
+  if (rc == PACI_OK && Gbias != nullptr) rc = colsum(dtype, mu * T, 3 * H * dh, dqkv, Gbias, s);
+  return rc;
 }
 
 size_t attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh) {
@@ -114,7 +123,7 @@ int paci_op_attention_fwd(int dtype, int mu, int T, int H, int dh, const void* q
 }
 int paci_op_attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
                           const void* o, const float* lse, void* dqkv, float* scratch, void* stream) {
-  return attention_bwd(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, (cudaStream_t)stream);
+  return attention_bwd(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, nullptr, (cudaStream_t)stream);
 }
 size_t paci_op_attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh) {
   return attention_bwd_scratch_bytes(dtype, mu, T, H, dh);

@@ -435,8 +435,7 @@ static int backward_impl(paci_stage* st, char* slot, const void* dout, void* din
     RC(gemm(dt, 2, D, D, M, st->sc_dx1, D, slot + b.o, D, nullptr, wo.g, D, 1, cs));
     // a17: attention backward
     RC(attention_bwd(dt, st->mu, st->T, st->H, st->dh, st->sc_dD2, slot + b.qkv, slot + b.o,
-                     (float*)(slot + b.lse), st->sc_dqkv, st->sc_attn, cs));
-    RC(colsum(dt, M, 3 * D, st->sc_dqkv, bqkv.g, cs));
+                     (float*)(slot + b.lse), st->sc_dqkv, st->sc_attn, bqkv.g, cs));   // + G_bqkv (a15)
     // QKV: dy1 = dqkv Wqkv ; G_Wqkv += dqkv^T y1
     RC(gemm(dt, 1, M, D, 3 * D, st->sc_dqkv, 3 * D, wqkv.wc, D, nullptr, st->sc_dD, D, 0, cs));
     RC(gemm(dt, 2, 3 * D, D, M, st->sc_dqkv, 3 * D, slot + b.y1, D, nullptr, wqkv.g, D, 1, cs));
