@@ -108,6 +108,18 @@ __device__ __forceinline__ float warp_max(float v) {
   return v;
 }
 
+// GELU (tanh form, R12) of the bf16 path: MUFU.TANH (max abs error ~5e-4, below the bf16 rounding
+// of the result).  Shared by gelu_fwd_kernel and the fused MLP-up GEMM epilogue so both give the same bits.
+__device__ __forceinline__ float tanh_fast(float u) {
+  float r;
+  asm("tanh.approx.f32 %0, %1;" : "=f"(r) : "f"(u));
+  return r;
+}
+__device__ __forceinline__ float gelu_bf16(float p) {
+  const float u = 0.7978845608028654f * (p + 0.044715f * p * p * p);
+  return 0.5f * p * (1.f + tanh_fast(u));
+}
+
 static inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 static inline size_t align_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
 
@@ -154,7 +166,11 @@ int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, con
 int gemm_simt(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
               const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s);
 int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
-            void* C, int ldc, int out_f32_accum, cudaStream_t s);
+            void* C, int ldc, int out_f32_accum, cudaStream_t s, void* gelu_out = nullptr);
+// C = A B^T + bias (pre-activation, stashed for backward) and Gout = gelu(C), both [M, N] with row stride ldc:
+// one launch on the tcgen05 path (GELU in the GEMM epilogue, rows a7 + a8), GEMM then gelu_fwd otherwise.
+int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
+                   void* C, void* Gout, int ldc, cudaStream_t s);
 bool gemm_backend_tcgen05();
 int add_vec(int dtype, size_t n, const void* a, const void* b, void* out, cudaStream_t s);  // out = a (+ b)
 

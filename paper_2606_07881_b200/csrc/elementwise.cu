@@ -326,11 +326,7 @@ int ln_bwd(int dtype, int rows, int D, const void* dy, const void* x, const floa
 // tanh: accurate tanhf in fp32 mode (1e-5 parity gate); in bf16 mode the single-instruction MUFU.TANH
 // (max abs error ~5e-4, below the bf16 rounding of the result) keeps the kernels HBM-bound, not ALU-bound.
 template <typename T> __device__ __forceinline__ float tanh_t(float u) { return tanhf(u); }
-template <> __device__ __forceinline__ float tanh_t<bf16>(float u) {
-  float r;
-  asm("tanh.approx.f32 %0, %1;" : "=f"(r) : "f"(u));
-  return r;
-}
+template <> __device__ __forceinline__ float tanh_t<bf16>(float u) { return tanh_fast(u); }
 template <typename T> __device__ __forceinline__ float gelu_f(float p) {
   const float u = GELU_C * (p + GELU_A * p * p * p);
   return 0.5f * p * (1.f + tanh_t<T>(u));

@@ -46,6 +46,7 @@ struct Params {
   int tiles_m, tiles_n, splits, kb_total;
   const float* bias;
   void* C;
+  int gelu;       // !ACCUM only: also store gelu(C) through tmC2 (MLP-up: the pre-activation is stashed, rows a7 + a8)
 };
 
 // ------------------------------------------------------------------ the kernel
@@ -55,7 +56,7 @@ struct Params {
 template <int CG, int BLOCK_N, int STAGES, bool A_MN, bool B_MN, bool ACCUM>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
 gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-               const __grid_constant__ CUtensorMap tmC, const Params p) {
+               const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmC2, const Params p) {
   constexpr int BN_CTA = BLOCK_N / CG;                  // B rows staged by one CTA
   constexpr uint32_t A_BYTES = BLOCK_M * BLOCK_K * 2, B_BYTES = BN_CTA * BLOCK_K * 2;
   constexpr uint32_t STAGE_BYTES = A_BYTES + B_BYTES;
@@ -223,9 +224,11 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 #pragma unroll 1
       for (int c = 0; c < BLOCK_N; c += CHUNK) {
         if (n0 + c >= p.N) break;                     // warp-uniform
-        uint8_t* buf = my_stage + sbuf * 4096;
-        sbuf ^= 1;
-        if (lane == 0) bulk_wait_read<1>();           // the box stored from this buffer two chunks ago is read
+        const bool gelu = !ACCUM && p.gelu != 0;       // kernel-uniform
+        uint8_t* buf = gelu ? my_stage : my_stage + sbuf * 4096;
+        uint8_t* buf2 = my_stage + 4096;               // gelu: second output tile of the same chunk
+        if (!gelu) sbuf ^= 1;
+        if (lane == 0) { if (gelu) bulk_wait_read<0>(); else bulk_wait_read<1>(); }   // staging buffer(s) free again
         __syncwarp();
         uint8_t* rowp = buf + lane * 128;
         if (ACCUM) {
@@ -243,11 +246,20 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
             for (int i = 0; i < 4; ++i) {
               const float4 b0 = *reinterpret_cast<const float4*>(my_bias + c + 32 * h + 8 * i);
               const float4 b1 = *reinterpret_cast<const float4*>(my_bias + c + 32 * h + 8 * i + 4);
-              const uint32_t w0 = pack_bf16x2(__uint_as_float(r[8 * i]) + b0.x, __uint_as_float(r[8 * i + 1]) + b0.y);
-              const uint32_t w1 = pack_bf16x2(__uint_as_float(r[8 * i + 2]) + b0.z, __uint_as_float(r[8 * i + 3]) + b0.w);
-              const uint32_t w2 = pack_bf16x2(__uint_as_float(r[8 * i + 4]) + b1.x, __uint_as_float(r[8 * i + 5]) + b1.y);
-              const uint32_t w3 = pack_bf16x2(__uint_as_float(r[8 * i + 6]) + b1.z, __uint_as_float(r[8 * i + 7]) + b1.w);
-              sts128(rowp + (((4 * h + i) ^ (lane & 7)) << 4), w0, w1, w2, w3);
+              uint32_t w[4];
+              w[0] = pack_bf16x2(__uint_as_float(r[8 * i]) + b0.x, __uint_as_float(r[8 * i + 1]) + b0.y);
+              w[1] = pack_bf16x2(__uint_as_float(r[8 * i + 2]) + b0.z, __uint_as_float(r[8 * i + 3]) + b0.w);
+              w[2] = pack_bf16x2(__uint_as_float(r[8 * i + 4]) + b1.x, __uint_as_float(r[8 * i + 5]) + b1.y);
+              w[3] = pack_bf16x2(__uint_as_float(r[8 * i + 6]) + b1.z, __uint_as_float(r[8 * i + 7]) + b1.w);
+              const uint32_t off = (uint32_t)(((4 * h + i) ^ (lane & 7)) << 4);
+              sts128(rowp + off, w[0], w[1], w[2], w[3]);
+              if (gelu) {                              // gelu of the ROUNDED pre-activation, as backward will see it
+                uint32_t gw[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                  gw[u] = pack_bf16x2(gelu_bf16(__uint_as_float(w[u] << 16)), gelu_bf16(__uint_as_float(w[u] & 0xffff0000u)));
+                sts128(buf2 + lane * 128 + off, gw[0], gw[1], gw[2], gw[3]);
+              }
             }
           }
         }
@@ -256,6 +268,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         if (lane == 0) {
           if (ACCUM) tma_reduce_add_2d(&tmC, buf, n0 + c, m0 + q * 32);
           else tma_store_2d(&tmC, buf, n0 + c, m0 + q * 32);
+          if (gelu) tma_store_2d(&tmC2, buf2, n0 + c, m0 + q * 32);
           bulk_commit();
         }
       }
@@ -346,8 +359,8 @@ int make_map(CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64
 
 
 template <int CG, int BLOCK_N, int STAGES, bool A_MN, bool B_MN, bool ACCUM>
-int launch(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmC, const Params& p, int grid,
-           cudaStream_t s) {
+int launch(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmC, const CUtensorMap& tmC2,
+           const Params& p, int grid, cudaStream_t s) {
   constexpr size_t SMEM = (size_t)STAGES * (BLOCK_M * BLOCK_K * 2 + (BLOCK_N / CG) * BLOCK_K * 2) +
                           EPI_STAGING_BYTES + 4 * BLOCK_N * 4 + 1024 + 256;
   static_assert(SMEM <= 232448, "shared memory budget of one sm_100 CTA");
@@ -369,7 +382,7 @@ int launch(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tm
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  PACI_CUDA_OK(cudaLaunchKernelEx(&cfg, kern, tmA, tmB, tmC, p));
+  PACI_CUDA_OK(cudaLaunchKernelEx(&cfg, kern, tmA, tmB, tmC, tmC2, p));
   g_launches.fetch_add(1, std::memory_order_relaxed);
   return PACI_OK;
 }
@@ -391,8 +404,10 @@ int make_tensor_map(CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1,
 }
 
 int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
-            void* C, int ldc, int out_f32_accum, cudaStream_t s) {
+            void* C, int ldc, int out_f32_accum, cudaStream_t s, void* gelu_out) {
   if (M <= 0 || N <= 0) return PACI_OK;
+  if (gelu_out != nullptr && (out_f32_accum || (uintptr_t)gelu_out % 16))
+    return fail(PACI_EINVAL, "tcgen05 GEMM: gelu output needs the bf16 epilogue and a 16-byte aligned pointer");
   if (K <= 0) return fail(PACI_EINVAL, "tcgen05 GEMM: K=%d", K);
   if (layout < 0 || layout > 2) return fail(PACI_EINVAL, "gemm: layout %d", layout);
   if ((uintptr_t)C % 16 || (out_f32_accum ? ldc % 4 : ldc % 8))
@@ -401,7 +416,7 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
   const bool a_mn = layout == 2, b_mn = layout != 0;
   const int CG = cta_group();
   const int BN = N <= 128 ? 128 : 256;
-  CUtensorMap tmA, tmB, tmC;
+  CUtensorMap tmA, tmB, tmC, tmC2;
   int rc;
   // A: K-major [M rows][K contiguous] -> dims {K, M}, box {64, 128};  MN-major [K rows][M contiguous] -> {M, K}, {64, 64}
   rc = a_mn ? make_map(&tmA, A, M, K, lda, 64, BLOCK_K) : make_map(&tmA, A, K, M, lda, BLOCK_K, BLOCK_M);
@@ -411,8 +426,10 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
   // C: box of 32 rows x 128 bytes, written by one epilogue warp per TMA store / reduce-add
   rc = out_f32_accum ? make_map(&tmC, C, N, M, ldc, 32, 32, 4) : make_map(&tmC, C, N, M, ldc, 64, 32, 2);
   if (rc) return rc;
+  tmC2 = tmC;
+  if (gelu_out != nullptr && (rc = make_map(&tmC2, gelu_out, N, M, ldc, 64, 32, 2))) return rc;
   Params p;
-  p.M = M; p.N = N; p.K = K; p.ldc = ldc; p.bias = bias; p.C = C;
+  p.M = M; p.N = N; p.K = K; p.ldc = ldc; p.bias = bias; p.C = C; p.gelu = gelu_out != nullptr;
   p.tiles_m = ceil_div(M, BLOCK_M * CG);
   p.tiles_n = ceil_div(N, BN);
   p.kb_total = ceil_div(K, BLOCK_K);
@@ -433,7 +450,7 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
   }
   p.splits = splits;
   const int grid = std::min(tiles * splits, workers) * CG;
-#define GO(CG_, BN_, ST_, AMN, BMN, ACC) return launch<CG_, BN_, ST_, AMN, BMN, ACC>(tmA, tmB, tmC, p, grid, s)
+#define GO(CG_, BN_, ST_, AMN, BMN, ACC) return launch<CG_, BN_, ST_, AMN, BMN, ACC>(tmA, tmB, tmC, tmC2, p, grid, s)
 #define BY_LAYOUT(CG_, BN_, ST_)                                                                          \
   do {                                                                                                    \
     if (out_f32_accum) {                                                                                  \

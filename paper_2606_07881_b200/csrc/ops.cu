@@ -39,6 +39,18 @@ int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, con
   return gemm_simt(dtype, layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, s);
 }
 
+int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
+                   void* C, void* Gout, int ldc, cudaStream_t s) {
+  if (dtype == PACI_BF16 && gemm_backend_tcgen05()) {
+    ProfScope prof(PC_GEMM_FWD, 2.0 * M * N * K, 2.0 * ((double)M * K + (double)N * K) + 4.0 * M * N, s);
+    return gemm_tc(0, M, N, K, A, lda, B, ldb, bias, C, ldc, 0, s, Gout);
+  }
+  int rc = gemm(dtype, 0, M, N, K, A, lda, B, ldb, bias, C, ldc, 0, s);
+  if (rc != PACI_OK) return rc;
+  if (ldc != N) return fail(PACI_EINVAL, "gemm_bias_gelu: the unfused path needs ldc == N");
+  return gelu_fwd(dtype, (size_t)M * N, C, Gout, s);
+}
+
 int attention_fwd_mma(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
 int attention_fwd_tc(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
 int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
