@@ -425,7 +425,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", default="medium", choices=sorted(CONFIGS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--sample-stride", type=int, default=41,
+    ap.add_argument("--sample-stride", type=int, default=97,
                     help="time every n-th library op with CUDA events; a sampled op runs alone on the GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stage-times", action="store_true")

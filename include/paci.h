@@ -189,6 +189,12 @@ int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_
  * PACI_BF16: all leading dimensions and pointers must be multiples of 8 elements / 16 bytes. */
 int paci_op_gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
                  const float* bias, void* C, int ldc, int out_f32_accum, void* stream);
+/* MLP-up with the activation fused (rows a7 + a8):  C = A B^T + bias (the pre-activation, which backward needs)
+ * and G = gelu(C), both [M, N] of T with row stride ldc, A[M,K], B[N,K] row-major.  PACI_BF16 on the tcgen05 path:
+ * ONE launch, gelu of the rounded C is computed in the GEMM epilogue and leaves through a second TMA store;
+ * otherwise the GEMM followed by the GELU kernel (needs ldc == N). */
+int paci_op_gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
+                           const float* bias, void* C, void* G, int ldc, void* stream);
 /* y = LN(x (+ res)) with gain g, bias b (fp32 [D]); writes xsum = x + res if xsum != NULL, and
  * mean, rstd (fp32 [rows]).  (a2, a6) */
 int paci_op_layernorm_fwd(int dtype, int rows, int D, const void* x, const void* res, const float* g,

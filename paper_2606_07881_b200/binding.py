@@ -65,6 +65,7 @@ SIGNATURES = {
     "paci_pipeline_destroy": (_i, [_vp]),
     "paci_pipeline_run": (_i, [_vp, _vp, C.c_int32, _i64, C.c_int32, _f, C.POINTER(RunReport)]),
     "paci_op_gemm": (_i, [_i, _i, _i, _i, _i, _vp, _i, _vp, _i, _vp, _vp, _i, _i, _vp]),
+    "paci_op_gemm_bias_gelu": (_i, [_i, _i, _i, _i, _vp, _i, _vp, _i, _vp, _vp, _vp, _i, _vp]),
     "paci_op_layernorm_fwd": (_i, [_i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_layernorm_bwd": (_i, [_i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_gelu_fwd": (_i, [_i, _sz, _vp, _vp, _vp]),

@@ -110,6 +110,10 @@ int paci_op_gemm(int dtype, int layout, int M, int N, int K, const void* A, int 
                  const float* bias, void* C, int ldc, int out_f32_accum, void* stream) {
   return gemm(dtype, layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, (cudaStream_t)stream);
 }
+int paci_op_gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
+                           const float* bias, void* C, void* G, int ldc, void* stream) {
+  return gemm_bias_gelu(dtype, M, N, K, A, lda, B, ldb, bias, C, G, ldc, (cudaStream_t)stream);
+}
 int paci_op_layernorm_fwd(int dtype, int rows, int D, const void* x, const void* res, const float* g,
                           const float* b, void* xsum, void* y, float* mean, float* rstd, void* stream) {
   return ln_fwd(dtype, rows, D, x, res, g, b, xsum, y, mean, rstd, (cudaStream_t)stream);

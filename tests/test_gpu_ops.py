@@ -90,6 +90,23 @@ def test_layernorm_fwd_bwd(dtype, rows, D):
     assert rel_l2(host(Gc) - 1.0, host(dx).sum(0)) < 1e-5            # column sums of what was stored
 
 
+@pytest.mark.parametrize("dtype,M,N,K", [(pb.FP32, 70, 96, 40), (pb.BF16, 300, 328, 192), (pb.BF16, 512, 1024, 256)])
+def test_gemm_bias_gelu(dtype, M, N, K):
+    """MLP-up with the activation in the GEMM epilogue (bf16: one tcgen05 launch, two TMA-stored tiles):
+    pre-activation and gelu(pre-activation) against the oracle, ragged M / N tails included."""
+    rng = np.random.default_rng(M + N)
+    x, W, b = rng.standard_normal((M, K)), rng.standard_normal((N, K)) * 0.2, rng.standard_normal(N)
+    xr, Wr = rounded(x, dtype), rounded(W, dtype)
+    p_ref = model.linear_fwd(xr, Wr, b.astype(np.float32).astype(np.float64))
+    Cd = torch.empty(M, N, device="cuda", dtype=DT[dtype])
+    Gd = torch.empty(M, N, device="cuda", dtype=DT[dtype])
+    ck(lib.paci_op_gemm_bias_gelu(dtype, M, N, K, dev(x, dtype).data_ptr(), K, dev(W, dtype).data_ptr(), K,
+                                  f32(b).data_ptr(), Cd.data_ptr(), Gd.data_ptr(), N, S0))
+    assert rel_l2(host(Cd), p_ref) < TOL[dtype] / 4
+    assert rel_l2(host(Gd), model.gelu_fwd(host(Cd))) < TOL[dtype] / 4      # gelu of what was stored
+    assert rel_l2(host(Gd), model.gelu_fwd(p_ref)) < TOL[dtype] / 2
+
+
 @pytest.mark.parametrize("dtype", BOTH)
 def test_gelu_fwd_bwd_colsum(dtype):
     rng = np.random.default_rng(5)
