@@ -371,7 +371,7 @@ __device__ __forceinline__ void red_add_v4(float* dst, float a, float b, float c
   asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 template <typename T, bool GELU>
-__global__ void __launch_bounds__(CS_TX * CS_TY) colslab_kernel(int rows, int cols, const T* __restrict__ a,
+__global__ void __launch_bounds__(CS_TX * CS_TY, 2) colslab_kernel(int rows, int cols, const T* __restrict__ a,
                                                                  const T* __restrict__ p, T* __restrict__ out,
                                                                  float* __restrict__ G) {
   constexpr int V = Vec<T>::N;
@@ -389,29 +389,33 @@ __global__ void __launch_bounds__(CS_TX * CS_TY) colslab_kernel(int rows, int co
   const int stride = gridDim.y * CS_TY;
   if (live) {
     for (int r0 = blockIdx.y * CS_TY + ty; r0 < rows; r0 += CS_U * stride) {
-      float v[CS_U][V], pv[CS_U][V];
+      uint4 rv[CS_U], rp[CS_U];                        // packed: 8 registers per row instead of 2 V
 #pragma unroll
       for (int u = 0; u < CS_U; ++u) {
         const int r = r0 + u * stride;
         if (r < rows) {
           const size_t off = (size_t)r * cols + c;
-          load_vec<T>(a + off, v[u]);
-          if (GELU) load_vec<T>(p + off, pv[u]);
+          rv[u] = load_raw<T>(a + off);
+          if (GELU) rp[u] = load_raw<T>(p + off);
         }
       }
 #pragma unroll
       for (int u = 0; u < CS_U; ++u) {
         const int r = r0 + u * stride;
         if (r < rows) {
+          float v[V];
+          unpack_raw<T>(rv[u], v);
           if (GELU) {
+            float pv[V];
+            unpack_raw<T>(rp[u], pv);
 #pragma unroll
-            for (int j = 0; j < V; ++j) v[u][j] *= dgelu_f<T>(pv[u][j]);
-            store_vec<T>(out + (size_t)r * cols + c, v[u]);
+            for (int j = 0; j < V; ++j) v[j] *= dgelu_f<T>(pv[j]);
+            store_vec<T>(out + (size_t)r * cols + c, v);
 #pragma unroll
-            for (int j = 0; j < V; ++j) v[u][j] = to_f(from_f<T>(v[u][j]));  // sum what was stored
+            for (int j = 0; j < V; ++j) v[j] = to_f(from_f<T>(v[j]));  // sum what was stored
           }
 #pragma unroll
-          for (int j = 0; j < V; ++j) acc[j] += v[u][j];
+          for (int j = 0; j < V; ++j) acc[j] += v[j];
         }
       }
     }

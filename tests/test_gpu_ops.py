@@ -97,7 +97,7 @@ def test_gemm_bias_gelu(dtype, M, N, K):
     rng = np.random.default_rng(M + N)
     x, W, b = rng.standard_normal((M, K)), rng.standard_normal((N, K)) * 0.2, rng.standard_normal(N)
     xr, Wr = rounded(x, dtype), rounded(W, dtype)
-    p_ref = model.linear_fwd(xr, Wr, b.astype(np.float32).astype(np.float64))
+    p_ref, _ = model.linear_fwd(xr, Wr, b.astype(np.float32).astype(np.float64))
     Cd = torch.empty(M, N, device="cuda", dtype=DT[dtype])
     Gd = torch.empty(M, N, device="cuda", dtype=DT[dtype])
     ck(lib.paci_op_gemm_bias_gelu(dtype, M, N, K, dev(x, dtype).data_ptr(), K, dev(W, dtype).data_ptr(), K,
