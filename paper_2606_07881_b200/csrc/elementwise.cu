@@ -32,6 +32,10 @@ int num_sms() {
   return n;
 }
 
+__device__ __forceinline__ void red_add_v4(float* dst, float a, float b, float c, float d) {
+  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
 static constexpr float LN_EPS = 1e-5f;              // DESIGN.md R13
 static constexpr float GELU_C = 0.7978845608028654f;  // sqrt(2/pi), R12
 static constexpr float GELU_A = 0.044715f;
@@ -222,7 +226,7 @@ __global__ void __launch_bounds__(LNC_TX * LNC_TY, 3) ln_bwd_cols_kernel(int row
                                                                        const T* __restrict__ dx, float* __restrict__ Gg,
                                                                        float* __restrict__ Gb, float* __restrict__ Gcol) {
   constexpr int V = Vec<T>::N;
-  __shared__ float red[3][LNC_TX * V];
+  __shared__ __align__(16) float red[3][LNC_TX * V];
   const int tx = threadIdx.x, ty = threadIdx.y;
   const int c = (blockIdx.x * LNC_TX + tx) * V;
   const bool live = c < D;
@@ -276,12 +280,13 @@ __global__ void __launch_bounds__(LNC_TX * LNC_TY, 3) ln_bwd_cols_kernel(int row
     }
   }
   __syncthreads();
-  for (int i = ty * LNC_TX + tx; i < LNC_TX * V; i += LNC_TX * LNC_TY) {
+  // one vector atomic per 4 columns per block (D % 4 == 0, G tensors are 16-byte aligned in the arena)
+  for (int i = (ty * LNC_TX + tx) * 4; i < LNC_TX * V; i += LNC_TX * LNC_TY * 4) {
     const int col = blockIdx.x * LNC_TX * V + i;
     if (col < D) {
-      atomicAdd(&Gg[col], red[0][i]);
-      atomicAdd(&Gb[col], red[1][i]);
-      if (Gcol != nullptr) atomicAdd(&Gcol[col], red[2][i]);
+      red_add_v4(Gg + col, red[0][i], red[0][i + 1], red[0][i + 2], red[0][i + 3]);
+      red_add_v4(Gb + col, red[1][i], red[1][i + 1], red[1][i + 2], red[1][i + 3]);
+      if (Gcol != nullptr) red_add_v4(Gcol + col, red[2][i], red[2][i + 1], red[2][i + 2], red[2][i + 3]);
     }
   }
 }
@@ -367,9 +372,6 @@ int gelu_fwd(int dtype, size_t n, const void* p, void* out, cudaStream_t s) {
 // ends with ONE vector atomic (red.global.add.v4.f32) per 4 columns.  (One scalar atomic per column per
 // 128-thread block put ~3000 serialized L2 atomics on every 32-byte sector of G: 0.15 of HBM peak.)
 constexpr int CS_TX = 64, CS_TY = 8, CS_U = 4;
-__device__ __forceinline__ void red_add_v4(float* dst, float a, float b, float c, float d) {
-  asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
-}
 template <typename T, bool GELU>
 __global__ void __launch_bounds__(CS_TX * CS_TY, 2) colslab_kernel(int rows, int cols, const T* __restrict__ a,
                                                                  const T* __restrict__ p, T* __restrict__ out,
