@@ -124,8 +124,8 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
   uint8_t* sP = sV + 2 * TILE_BYTES;
   uint64_t* bars = (uint64_t*)(sP + 2 * TILE_BYTES);
   uint64_t *q_full = bars, *k_full = bars + 1, *v_full = bars + 3, *k_empty = bars + 5, *v_empty = bars + 7,
-           *s_full = bars + 9, *p_full = bars + 10, *o_full = bars + 11;
-  uint32_t* tmem_slot = (uint32_t*)(bars + 12);
+           *s_full = bars + 9, *p_full = bars + 10, *o_full = bars + 11, *s_free = bars + 12;
+  uint32_t* tmem_slot = (uint32_t*)(bars + 13);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int D = H * DH;
@@ -141,7 +141,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
   if (threadIdx.x == 0) {
     mbar_init(q_full, 1);
     for (int i = 0; i < 2; ++i) { mbar_init(&k_full[i], 1); mbar_init(&v_full[i], 1); mbar_init(&k_empty[i], 1); mbar_init(&v_empty[i], 1); }
-    mbar_init(s_full, 1); mbar_init(p_full, 128); mbar_init(o_full, 1);
+    mbar_init(s_full, 1); mbar_init(p_full, 128); mbar_init(o_full, 1); mbar_init(s_free, 128);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -189,9 +189,13 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
       mbar_wait(q_full, 0, 14);
       issue_qk(0);
       for (int j = 0; j < n_kb; ++j) {
-        mbar_wait(p_full, (uint32_t)j & 1u, 15);           // P_j is in shared memory and S_j has been consumed
+        if (j + 1 < n_kb) {                                // S_j sits in the softmax threads' registers: the next
+          mbar_wait(s_free, (uint32_t)j & 1u, 20);          // scores are computed WHILE they do exp2 / pack
+          tc_fence_after();
+          issue_qk(j + 1);
+        }
+        mbar_wait(p_full, (uint32_t)j & 1u, 15);           // P_j is in shared memory
         tc_fence_after();
-        if (j + 1 < n_kb) issue_qk(j + 1);
         const int st = j & 1;
         mbar_wait(&v_full[st], (uint32_t)(j >> 1) & 1u, 16);
         tc_fence_after();
@@ -217,6 +221,8 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
 #pragma unroll
       for (int q = 0; q < 4; ++q) tmem_ld32_nowait(tS + lane_off + q * 32, s + q * 32);
       tmem_ld_wait();
+      tc_fence_before();
+      mbar_arrive(s_free);                                // S may be overwritten by Q K_{j+1}^T
       const bool diag = j == n_kb - 1;
       float mx = -INFINITY;
 #pragma unroll
@@ -245,6 +251,9 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
         }
         tmem_st_wait();
       }
+      // P is single-buffered: P_{j-1} V_{j-1} must have retired before P_j overwrites it (the next scores are
+      // ready early now, so this is no longer implied by the MMA issue order)
+      if (j > 0) { mbar_wait_many(o_full, (uint32_t)(j - 1) & 1u, 30); tc_fence_after(); }
       float sum = 0.f;
 #pragma unroll
       for (int ch = 0; ch < 16; ++ch) {                   // 16 chunks of 8 keys = 16 bytes of bf16
@@ -338,8 +347,8 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   uint8_t* sStat = sE1 + (DKDV ? 2 : 1) * TILE_BYTES;    // per stage: lse2[64], delta[64] of the streamed rows
   uint64_t* bars = (uint64_t*)(sStat + NST * 512);
   uint64_t *x_full = bars, *y_full = bars + 1, *y_empty = bars + 1 + NST, *t_full = bars + 1 + 2 * NST, *e_full = t_full + 1,
-           *e_empty = t_full + 2, *acc_full = t_full + 3;
-  uint32_t* tmem_slot = (uint32_t*)(t_full + 4);
+           *e_empty = t_full + 2, *acc_full = t_full + 3, *t_free = t_full + 4;
+  uint32_t* tmem_slot = (uint32_t*)(t_full + 5);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int D = H * DH;
@@ -359,7 +368,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   if (threadIdx.x == 0) {
     mbar_init(x_full, 1);
     for (int i = 0; i < NST; ++i) { mbar_init(&y_full[i], 1); mbar_init(&y_empty[i], 1); }
-    mbar_init(t_full, 1); mbar_init(e_full, 128 * EW); mbar_init(e_empty, 1); mbar_init(acc_full, 1);
+    mbar_init(t_full, 1); mbar_init(e_full, 128 * EW); mbar_init(e_empty, 1); mbar_init(acc_full, 1); mbar_init(t_free, 128 * EW);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -417,9 +426,13 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       mbar_wait(x_full, 0, 23);
       issue_t(0);
       for (int t = 0; t < n_steps; ++t) {
-        mbar_wait(e_full, (uint32_t)t & 1u, 24);          // E_t is in shared memory and T_t has been consumed
+        if (t + 1 < n_steps) {                            // T_t sits in the elementwise threads' registers: the next
+          mbar_wait(t_free, (uint32_t)t & 1u, 29);         // score-type MMAs run WHILE they do exp2 / pack
+          tc_fence_after();
+          issue_t(t + 1);
+        }
+        mbar_wait(e_full, (uint32_t)t & 1u, 24);          // E_t is in shared memory
         tc_fence_after();
-        if (t + 1 < n_steps) issue_t(t + 1);
         const int st = t % NST;
         const uint32_t aY0 = smem_u32(sY + st * YST), aY1 = aY0 + HALF_BYTES;
         const uint32_t acc = t > 0 ? 1u : 0u;
@@ -469,6 +482,8 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       tmem_ld_cols_nowait<CW>(tT0 + lane_off + cw0, s);
       tmem_ld_cols_nowait<CW>(tT1 + lane_off + cw0, dp);
       tmem_ld_wait();
+      tc_fence_before();
+      mbar_arrive(t_free);                                // T0 / T1 may be overwritten by step t+1's MMAs
       TICK(1);
       const float4* pl = reinterpret_cast<const float4*>(sStat + st * 512) + cw0 / 4;   // lse2 of the step's 64 queries
       const float4* pd = pl + 16;                                                        // delta
