@@ -436,16 +436,19 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
   const int tiles = p.tiles_m * p.tiles_n, workers = std::max(1, num_sms() / CG);
   int splits = 1;
   if (out_f32_accum) {
-    // split-K over the contraction (tokens): partials meet in the fp32 red.add epilogue.  Pick the split
-    // count that fills whole rounds of the persistent grid best (fewest splits on a tie).
+    // split-K over the contraction (tokens): partials meet in the fp32 TMA reduce-add epilogue.  Cost model in
+    // k-block units: rounds of the persistent grid x (k-blocks per item + EPI), where EPI ~ 8 k-blocks stands
+    // for an item's reduce-add epilogue (every extra split re-sends the whole fp32 tile through the L2 adders:
+    // 8 splits of the 4096x1024 wgrad measured 73 us against 1 split's 1.73-round quantisation loss).
     const int max_s = std::max(1, std::min(p.kb_total / 4, 32));
-    double best = -1.0;
+    const int EPI = 8;
+    long best = -1;
     for (int sp = 1; sp <= max_s; ++sp) {
       const int kb_per = ceil_div(p.kb_total, sp);
       if (ceil_div(p.kb_total, kb_per) != sp) continue;        // every split owns at least one k-block
-      const long items = (long)tiles * sp;
-      const double eff = (double)items / ((double)ceil_div(items, workers) * workers);
-      if (eff > best + 0.02) { best = eff; splits = sp; }
+      const long rounds = ceil_div((long)tiles * sp, workers);
+      const long cost = rounds * (kb_per + EPI);
+      if (best < 0 || cost < best) { best = cost; splits = sp; }
     }
   }
   p.splits = splits;
