@@ -217,9 +217,11 @@ __global__ void __launch_bounds__(256, 3) ln_bwd_dx_kernel(int rows, int D, cons
   }
 }
 
-constexpr int LNC_TX = 128, LNC_TY = 2, LNC_U = 4;
+// 1024-thread blocks, one per SM: every column then receives only ~148 global atomics (444 small blocks put 444
+// serialized L2 atomics on each 16-byte address, which cost more than streaming the 50 MB)
+constexpr int LNC_TX = 128, LNC_TY = 8, LNC_U = 2;
 template <typename T>
-__global__ void __launch_bounds__(LNC_TX * LNC_TY, 3) ln_bwd_cols_kernel(int rows, int D, const T* __restrict__ dy,
+__global__ void __launch_bounds__(LNC_TX * LNC_TY, 1) ln_bwd_cols_kernel(int rows, int D, const T* __restrict__ dy,
                                                                        const T* __restrict__ x,
                                                                        const float* __restrict__ mean,
                                                                        const float* __restrict__ rstd,
@@ -311,7 +313,7 @@ static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float*
   }
 #undef LNB_CASE
   const int gx = ceil_div(D / V, LNC_TX);
-  int gy = std::max(1, 3 * num_sms() / gx);
+  int gy = std::max(1, num_sms() / gx);
   gy = std::min(gy, ceil_div(rows, LNC_TY));
   PACI_LAUNCH((ln_bwd_cols_kernel<T>), dim3(gx, gy), dim3(LNC_TX, LNC_TY), 0, s, rows, D, (const T*)dy,
               (const T*)x, mean, rstd, (const T*)dx, Gg, Gb, Gcol);
