@@ -293,12 +293,122 @@ __global__ void __launch_bounds__(LNC_TX * LNC_TY, 1) ln_bwd_cols_kernel(int row
   }
 }
 
+// Single-pass variant (D = NW x 32 x V, NW <= 8 warps per row): a block of NW warps owns a stream of rows and
+// handles LNF_R of them per iteration; a lane owns ONE 16-byte column vector, so the three column partials are
+// 3 V registers (not 3 D/32 as in a warp-per-row kernel) and dy, x, dres are read exactly once.  The row sums
+// mean(g dy), mean(g dy xhat) cross the NW warps through shared memory (one barrier per LNF_R rows, double-
+// buffered).  Per block, one vector atomic per 4 columns at the end.
+constexpr int LNF_R = 4;
+template <typename T, int NW>
+__global__ void __launch_bounds__(NW * 32) ln_bwd_fused_kernel(int rows, int D, const T* __restrict__ dy,
+                                                               const T* __restrict__ x, const float* __restrict__ mean,
+                                                               const float* __restrict__ rstd,
+                                                               const float* __restrict__ g, const T* __restrict__ dres,
+                                                               T* __restrict__ dx, float* __restrict__ Gg,
+                                                               float* __restrict__ Gb, float* __restrict__ Gcol) {
+  constexpr int V = Vec<T>::N;
+  __shared__ float part[2][LNF_R][2][NW];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int c = (w * 32 + lane) * V;                      // this lane's columns
+  float gg[V], ag[V], ab[V], ac[V];
+  load_f32<V>(g + c, gg);
+#pragma unroll
+  for (int j = 0; j < V; ++j) ag[j] = ab[j] = ac[j] = 0.f;
+  const float invD = 1.f / (float)D;
+  int buf = 0;
+  for (int r0 = blockIdx.x * LNF_R; r0 < rows; r0 += gridDim.x * LNF_R, buf ^= 1) {
+    uint4 rdy[LNF_R], rx[LNF_R], rr[LNF_R];
+    float mu[LNF_R], rs[LNF_R];
+#pragma unroll
+    for (int u = 0; u < LNF_R; ++u) {
+      const int r = r0 + u;
+      if (r < rows) {
+        const size_t off = (size_t)r * D + c;
+        rdy[u] = load_raw<T>(dy + off);
+        rx[u] = load_raw<T>(x + off);
+        if (dres != nullptr) rr[u] = load_raw<T>(dres + off);
+        mu[u] = __ldg(mean + r);
+        rs[u] = __ldg(rstd + r);
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < LNF_R; ++u) {
+      float s1 = 0.f, s2 = 0.f;
+      if (r0 + u < rows) {
+        float dyv[V], xv[V];
+        unpack_raw<T>(rdy[u], dyv);
+        unpack_raw<T>(rx[u], xv);
+#pragma unroll
+        for (int j = 0; j < V; ++j) {
+          const float gd = dyv[j] * gg[j];
+          s1 += gd;
+          s2 += gd * ((xv[j] - mu[u]) * rs[u]);
+        }
+      }
+      s1 = warp_sum(s1);
+      s2 = warp_sum(s2);
+      if (lane == 0) { part[buf][u][0][w] = s1; part[buf][u][1][w] = s2; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int u = 0; u < LNF_R; ++u) {
+      const int r = r0 + u;
+      if (r < rows) {
+        float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+        for (int k = 0; k < NW; ++k) { s1 += part[buf][u][0][k]; s2 += part[buf][u][1][k]; }
+        s1 *= invD;
+        s2 *= invD;
+        float dyv[V], xv[V], o[V];
+        unpack_raw<T>(rdy[u], dyv);
+        unpack_raw<T>(rx[u], xv);
+#pragma unroll
+        for (int j = 0; j < V; ++j) {
+          const float xh = (xv[j] - mu[u]) * rs[u];
+          o[j] = rs[u] * (dyv[j] * gg[j] - s1 - xh * s2);
+          ag[j] += dyv[j] * xh;
+          ab[j] += dyv[j];
+        }
+        if (dres != nullptr) {
+          float rv[V];
+          unpack_raw<T>(rr[u], rv);
+#pragma unroll
+          for (int j = 0; j < V; ++j) o[j] += rv[j];
+        }
+        store_vec<T>(dx + (size_t)r * D + c, o);
+        if (Gcol != nullptr) {
+#pragma unroll
+          for (int j = 0; j < V; ++j) ac[j] += to_f(from_f<T>(o[j]));   // sum of what was stored
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < V; j += 4) {
+    red_add_v4(Gg + c + j, ag[j], ag[j + 1], ag[j + 2], ag[j + 3]);
+    red_add_v4(Gb + c + j, ab[j], ab[j + 1], ab[j + 2], ab[j + 3]);
+    if (Gcol != nullptr) red_add_v4(Gcol + c + j, ac[j], ac[j + 1], ac[j + 2], ac[j + 3]);
+  }
+}
+
 template <typename T>
 static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float* mean, const float* rstd,
                     const float* g, const void* dres, void* dx, float* Gg, float* Gb, float* Gcol,
                     cudaStream_t s) {
   constexpr int V = Vec<T>::N;
   if (D % V != 0) return fail(PACI_EINVAL, "layernorm_bwd: D=%d not a multiple of %d", D, V);
+  if (D % (32 * V) == 0 && D / (32 * V) <= 8 && (uintptr_t)Gg % 16 == 0 && (uintptr_t)Gb % 16 == 0 &&
+      (Gcol == nullptr || (uintptr_t)Gcol % 16 == 0)) {
+    const int nw = D / (32 * V);
+    const int blocks = std::min(ceil_div(rows, LNF_R), num_sms() * std::max(1, 16 / nw));
+#define LNF_CASE(N)                                                                                      \
+  case N:                                                                                                \
+    PACI_LAUNCH((ln_bwd_fused_kernel<T, N>), blocks, N * 32, 0, s, rows, D, (const T*)dy, (const T*)x,  \
+                mean, rstd, g, (const T*)dres, (T*)dx, Gg, Gb, Gcol);                                    \
+    return PACI_OK;
+    switch (nw) { LNF_CASE(1) LNF_CASE(2) LNF_CASE(3) LNF_CASE(4) LNF_CASE(5) LNF_CASE(6) LNF_CASE(7) LNF_CASE(8) }
+#undef LNF_CASE
+  }
   const int nv = ceil_div(D / V, 32);
   const int wpb = 8;
   dim3 grid(ceil_div(rows, wpb)), block(wpb * 32);
