@@ -37,7 +37,10 @@ constexpr int BLOCK_M = 128;
 constexpr int BLOCK_K = 64;
 constexpr int UMMA_K = 16;
 constexpr int NUM_THREADS = 192;
-constexpr uint32_t EPI_STAGING_BYTES = 4 * 2 * 4096;
+constexpr int EPI_BUFS = 3;                 // staging boxes per epilogue warp: a box is reused only after the TMA store
+                                            // issued EPI_BUFS chunks ago has read it (2 buffers left ~0.7 us of store
+                                            // latency exposed per chunk: 3.1 us of epilogue for the last tile of a launch)
+constexpr uint32_t EPI_STAGING_BYTES = 4 * EPI_BUFS * 4096;
 
 using namespace tc;
 
@@ -69,7 +72,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
 
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint8_t* staging = smem + STAGES * STAGE_BYTES;        // 4 epilogue warps x 2 buffers x 4 KB (1024-aligned)
+  uint8_t* staging = smem + STAGES * STAGE_BYTES;        // 4 epilogue warps x EPI_BUFS buffers x 4 KB (1024-aligned)
   float* bias_s = (float*)(staging + EPI_STAGING_BYTES); // 4 epilogue warps x BLOCK_N floats
   uint64_t* full = (uint64_t*)(bias_s + 4 * BLOCK_N);
   uint64_t* empty = full + STAGES;
@@ -204,7 +207,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     // which makes the row-per-thread st.shared.v4 conflict-free.  TMA clips the box at the tensor edge.
     const int q = warp & 3;
     constexpr int CHUNK = ACCUM ? 32 : 64;            // columns per TMA box
-    uint8_t* my_stage = staging + (warp - 2) * 8192;
+    uint8_t* my_stage = staging + (warp - 2) * (EPI_BUFS * 4096);
     float* my_bias = bias_s + (warp - 2) * BLOCK_N;
     uint32_t acc = 0, acc_phase = 0, sbuf = 0;
     for (int item = worker; item < n_items; item += n_workers) {
@@ -227,8 +230,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         const bool gelu = !ACCUM && p.gelu != 0;       // kernel-uniform
         uint8_t* buf = gelu ? my_stage : my_stage + sbuf * 4096;
         uint8_t* buf2 = my_stage + 4096;               // gelu: second output tile of the same chunk
-        if (!gelu) sbuf ^= 1;
-        if (lane == 0) { if (gelu) bulk_wait_read<0>(); else bulk_wait_read<1>(); }   // staging buffer(s) free again
+        if (!gelu) sbuf = sbuf + 1 == EPI_BUFS ? 0 : sbuf + 1;
+        if (lane == 0) { if (gelu) bulk_wait_read<0>(); else bulk_wait_read<EPI_BUFS - 1>(); }   // staging buffer(s) free again
         __syncwarp();
         uint8_t* rowp = buf + lane * 128;
         if (ACCUM) {
@@ -238,14 +241,22 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
           for (int i = 0; i < 8; ++i)
             sts128(rowp + ((i ^ (lane & 7)) << 4), r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
         } else {
+          uint32_t r64[64];                            // both halves of the chunk in flight before one wait
+          tmem_ld32_nowait(taddr + c, r64);
+          tmem_ld32_nowait(taddr + c + 32, r64 + 32);
+          // the chunk's 64 bias values go to registers up front: interleaved with the (volatile, memory-
+          // clobbering) st.shared they serialised into 8 load -> add -> store chains, 0.4 us per chunk
+          float4 bq[16];
+#pragma unroll
+          for (int k = 0; k < 16; ++k) bq[k] = *reinterpret_cast<const float4*>(my_bias + c + 4 * k);
+          tmem_ld_wait();
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
-            uint32_t r[32];
-            tmem_ld32(taddr + c + 32 * h, r);
+            const uint32_t* r = r64 + 32 * h;
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-              const float4 b0 = *reinterpret_cast<const float4*>(my_bias + c + 32 * h + 8 * i);
-              const float4 b1 = *reinterpret_cast<const float4*>(my_bias + c + 32 * h + 8 * i + 4);
+              const float4 b0 = bq[8 * h + 2 * i];
+              const float4 b1 = bq[8 * h + 2 * i + 1];
               uint32_t w[4];
               w[0] = pack_bf16x2(__uint_as_float(r[8 * i]) + b0.x, __uint_as_float(r[8 * i + 1]) + b0.y);
               w[1] = pack_bf16x2(__uint_as_float(r[8 * i + 2]) + b0.z, __uint_as_float(r[8 * i + 3]) + b0.w);
@@ -281,7 +292,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
       acc ^= 1;
       if (acc == 0) acc_phase ^= 1;
     }
-    if (lane == 0) bulk_wait_all();                   // smem must outlive the last TMA read
+    if (lane == 0) bulk_wait_read<0>();               // smem must outlive the last TMA read; the global writes are
+                                                      // complete at kernel end like any other store
   }
   tc_fence_before();
   __syncthreads();
