@@ -123,3 +123,21 @@ def test_stage_full_width_micro_batch_1(s, S, L):
         got = st.read(name, pb.GRAD_ACCUM)
         assert rel_l2(got, g) < TOL[pb.BF16], (name, rel_l2(got, g))
     st.close()
+
+
+def test_pipeline_full_width_with_drift():
+    """The schedule driver at GPT-2-Medium width (D 1024, H 16, T 1024, V 50257; 2 emulated stages x 1 block,
+    micro-batch 1, k = 2, 4 micro-batches): stage 0 crosses one update at micro-batch 2 (Eq. 8), so its backward
+    runs on stale activations with the updated weights (Eq. 1) through the tcgen05 GEMM / attention kernels and the
+    fused AdamW.  Counts and versions exact; losses and weights after two updates within the bf16 gates."""
+    from oracle import pipeline as opipe
+    from test_gpu_pipeline import _build, _compare
+    S, L, mu, k, n, lr = 2, 1, 1, 2, 4, 3e-4
+    specs, params, stages = _build(pb.BF16, S, L, D, H, T, mu, V, k, seed=7)
+    tok = synth.tokens(7, n, mu, T, V, "zipf")
+    ref = opipe.run_pipeline(specs, params, tok, k, lr)
+    assert ref["delta"][0] == [0, 0, 1, 0] and ref["version"] == [2, 2]
+    out = pb.Pipeline(stages).run(torch.from_numpy(tok).cuda(), lr)
+    _compare(out, ref, stages, pb.BF16, n, 5e-3, lr_bound=2 * lr)
+    for st in stages:
+        st.close()
