@@ -464,7 +464,11 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
     }
   }
   p.splits = splits;
-  const int grid = std::min(tiles * splits, workers) * CG;
+  // balanced persistent grid: the same number of rounds on the fewest workers (128 tiles on 74 pairs take 2
+  // rounds; so do 64 pairs, and the other 20 SMs stay free for the other stage streams' kernels)
+  const int items = tiles * splits;
+  const int rounds = ceil_div(items, workers);
+  const int grid = ceil_div(items, rounds) * CG;
 #define GO(CG_, BN_, ST_, AMN, BMN, ACC) return launch<CG_, BN_, ST_, AMN, BMN, ACC>(tmA, tmB, tmC, tmC2, p, grid, s)
 #define BY_LAYOUT(CG_, BN_, ST_)                                                                          \
   do {                                                                                                    \
