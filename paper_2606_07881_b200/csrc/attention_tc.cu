@@ -212,14 +212,20 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
       tc_fence_before();
       mbar_arrive(s_free);                                // S may be overwritten by Q K_{j+1}^T
       const bool diag = j == n_kb - 1;
-      float mx = -INFINITY;
+      // row max of the RAW scores with four independent chains (one chain of 128 dependent FMNMX costs ~500
+      // cycles); the scale c > 0 is applied to the max and folded into the exp2 argument as one FFMA
+      float mx4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+      if (diag) {
 #pragma unroll
-      for (int i = 0; i < 128; ++i) {
-        float v = __uint_as_float(s[i]) * c;
-        if (diag && i > r) v = -INFINITY;
-        s[i] = __float_as_uint(v);
-        mx = fmaxf(mx, v);
+        for (int i = 0; i < 128; ++i) {
+          if (i > r) s[i] = __float_as_uint(-INFINITY);
+          mx4[i & 3] = fmaxf(mx4[i & 3], __uint_as_float(s[i]));
+        }
+      } else {
+#pragma unroll
+        for (int i = 0; i < 128; ++i) mx4[i & 3] = fmaxf(mx4[i & 3], __uint_as_float(s[i]));
       }
+      const float mx = fmaxf(fmaxf(mx4[0], mx4[1]), fmaxf(mx4[2], mx4[3])) * c;
       // lazy rescale (warp-uniform branch: tcgen05.ld / st are warp-collective)
       const bool grow = mx > m_ref + 8.f;
       if (j == 0) {
@@ -242,20 +248,21 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
       // P is single-buffered: P_{j-1} V_{j-1} must have retired before P_j overwrites it (the next scores are
       // ready early now, so this is no longer implied by the MMA issue order)
       if (j > 0) { mbar_wait_many(o_full, (uint32_t)(j - 1) & 1u, 30); tc_fence_after(); }
-      float sum = 0.f;
+      float sum4[4] = {0.f, 0.f, 0.f, 0.f};
+      const float neg_m = -m_ref;
 #pragma unroll
       for (int ch = 0; ch < 16; ++ch) {                   // 16 chunks of 8 keys = 16 bytes of bf16
         uint32_t w[4];
 #pragma unroll
         for (int t = 0; t < 4; ++t) {
-          const float p0 = ex2(__uint_as_float(s[ch * 8 + 2 * t]) - m_ref);
-          const float p1 = ex2(__uint_as_float(s[ch * 8 + 2 * t + 1]) - m_ref);
-          sum += p0 + p1;
+          const float p0 = ex2(fmaf(__uint_as_float(s[ch * 8 + 2 * t]), c, neg_m));       // exp2(-inf) = 0: masked
+          const float p1 = ex2(fmaf(__uint_as_float(s[ch * 8 + 2 * t + 1]), c, neg_m));
+          sum4[t] += p0 + p1;
           w[t] = pack_bf16x2(p0, p1);
         }
         sts128(prow + (ch >> 3) * TILE_BYTES + (((ch & 7) ^ (r & 7)) << 4), w[0], w[1], w[2], w[3]);
       }
-      l += sum;
+      l += (sum4[0] + sum4[1]) + (sum4[2] + sum4[3]);
       fence_async_smem();                                 // P visible to the tensor core's async proxy
       tc_fence_before();
       mbar_arrive(p_full);
