@@ -2,15 +2,21 @@
 // Rows a3, a5, a7, a9, a10 (forward, "NT"), a12/a13 (dgrad with the CURRENT weights, "NN") and a14
 // (wgrad whose epilogue ADDS into the fp32 accumulator G, "TN", split-K over tokens) of SURVEY.md 8(a).
 //
-// Structure (one CTA per SM, persistent over work items, 192 threads):
-//   warp 0      TMA producer: cp.async.bulk.tensor 2D tiles -> 128B-swizzled shared memory, 4-stage ring
-//   warp 1      MMA issuer: one thread issues tcgen05.mma (M=128, N=BLOCK_N, K=16) from shared-memory
-//               matrix descriptors; accumulators live in TMEM (2 buffers x BLOCK_N fp32 columns), so the
-//               epilogue of tile i overlaps the main loop of tile i+1
-//   warps 2-5   epilogue: tcgen05.ld (32 lanes x 32 columns per warp) -> registers -> (+bias, ->bf16)
-//               st.global, or red.global.add.v4.f32 into the fp32 accumulator (beta = 1)
-// Pipelines: full/empty mbarriers between TMA and MMA (tcgen05.commit frees a stage), tmem_full /
-// tmem_empty between MMA and epilogue.
+// Structure: persistent, one CTA per SM, 192 threads; by default the two CTAs of a cluster (one TPC) work as a
+// PAIR on a 256 x 256 tile (tcgen05.mma.cta_group::2, M = 256): each CTA stages its own 128 rows of A and HALF of
+// the B tile, the leader issues the MMAs for both, each CTA keeps its 128 accumulator rows in its own TMEM.
+//   warp 0      TMA producer: cp.async.bulk.tensor 2D tiles -> 128B-swizzled shared memory, 5-stage ring; in pair
+//               mode both CTAs' bytes are counted on the LEADER's "full" mbarrier
+//   warp 1      MMA issuer (leader CTA only): one thread issues tcgen05.mma (N = BLOCK_N, K = 16) from shared-
+//               memory matrix descriptors; accumulators live in TMEM (2 buffers x BLOCK_N fp32 columns), so the
+//               epilogue of tile i overlaps the main loop of tile i+1; tcgen05.commit (multicast to both CTAs)
+//               frees a stage / publishes an accumulator
+//   warps 2-5   epilogue: tcgen05.ld (32 lanes x 64 columns per warp and chunk) -> (+bias from registers, ->bf16)
+//               -> 128B-swizzled staging box in shared memory -> TMA store, or, for the fp32 accumulator G
+//               (beta = 1, Alg. 1 line 13), TMA reduce-add (cp.reduce.async.bulk.tensor .add): wgrad accumulation
+//               and split-K partials are the same mechanism and need no separate kernel
+// Pipelines: full/empty mbarriers between TMA and MMA, tmem_full / tmem_empty between MMA and epilogue (the
+// peer's epilogue warps arrive on the leader's barrier through the cluster address space).
 //
 // Operand layouts.  "K-major" = contraction index contiguous in memory, "MN-major" = the other index
 // contiguous.  Both are staged by TMA with the 128-byte swizzle and described to the tensor core by a
