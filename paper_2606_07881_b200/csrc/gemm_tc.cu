@@ -227,7 +227,7 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
         }
         __syncwarp();
       }
-      mbar_wait(&tfull[acc], acc_phase, 4);
+      mbar_wait_many(&tfull[acc], acc_phase, 4);     // 128 threads wait a whole main loop: sleep between polls
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BLOCK_N;
 #pragma unroll 1
