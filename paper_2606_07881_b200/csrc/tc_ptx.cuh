@@ -173,24 +173,18 @@ __device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t* r) {
       : "r"(taddr));
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-// mbarrier wait for the 128..256 elementwise threads: after a few failed polls they sleep between polls, so
-// waiting warps do not take issue slots from the working warps of the other CTA on the SM.
+// mbarrier wait for the 128..256 elementwise / epilogue threads: try_wait with a suspend-time hint, so a waiting
+// warp is parked by the hardware until the phase completes (or ~1 us passes) instead of spinning through
+// try_wait / branch / yield -- spinning warps took about as many issue slots as the working warps' arithmetic.
 __device__ __forceinline__ void mbar_wait_many(uint64_t* bar, uint32_t parity, int tag) {
   const uint32_t addr = smem_u32(bar);
-  for (int i = 0; i < 4; ++i) {
-    uint32_t done;
-    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.b32 %0, 1, 0, p;\n\t}"
-                 : "=r"(done) : "r"(addr), "r"(parity) : "memory");
-    if (done) return;
-  }
   uint32_t spins = 0;
   uint64_t t0 = 0;
   while (true) {
     uint32_t done;
-    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.b32 %0, 1, 0, p;\n\t}"
-                 : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.b32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(addr), "r"(parity), "r"(1000u) : "memory");
     if (done) return;
-    __nanosleep(64);
     if ((++spins & 255u) == 0) {
       const uint64_t now = globaltimer_ns();
       if (t0 == 0) t0 = now;
