@@ -55,6 +55,24 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
         "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
       : "memory");
 }
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+      "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};"
+      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+        "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+      : "memory");
+}
+// tcgen05.mma with the A operand in TENSOR MEMORY (K-major only): lane = row, one 32-bit column = two bf16 of K
+__device__ __forceinline__ void umma_bf16_ts(uint32_t tmem_d, uint32_t tmem_a, uint64_t bdesc, uint32_t idesc_,
+                                             uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(tmem_d), "r"(tmem_a), "l"(bdesc), "r"(idesc_), "r"(accumulate)
+      : "memory");
+}
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ float ex2(float x) {
   float r;
@@ -285,10 +303,10 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
 constexpr int BWD_EW = 2;                               // elementwise warpgroups: each thread owns 64/EW columns
 constexpr int BWD_THREADS = 64 + 128 * BWD_EW;
 constexpr uint32_t HALF_BYTES = 64 * 128;               // 64 rows x 64 bf16
-// ring depth: DKDV needs both E tiles (P^T, dS^T) and fits 2 stages in half an SM's shared memory; DQ has one E tile and takes 3
-__host__ __device__ constexpr int bwd_stages(bool dkdv) { return dkdv ? 2 : 3; }
+// ring depth: DKDV keeps both E tiles (P^T, dS^T) in shared memory and fits 2 stages in half an SM; DQ (dS in TMEM) takes 4
+__host__ __device__ constexpr int bwd_stages(bool dkdv) { return dkdv ? 2 : 4; }
 __host__ __device__ constexpr uint32_t bwd_smem(bool dkdv) {
-  return 2 * TILE_BYTES + bwd_stages(dkdv) * (2 * HALF_BYTES + 512) + (dkdv ? 2u : 1u) * TILE_BYTES + 256;
+  return 2 * TILE_BYTES + bwd_stages(dkdv) * (2 * HALF_BYTES + 512) + (dkdv ? 2u : 0u) * TILE_BYTES + 256;   // DQ: dS lives in TMEM
 }
 
 __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
@@ -310,7 +328,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   constexpr int NST = bwd_stages(DKDV);
   uint8_t* sE1 = sY + NST * YST;
   uint8_t* sE0 = sE1 + TILE_BYTES;                       // DKDV only
-  uint8_t* sStat = sE1 + (DKDV ? 2 : 1) * TILE_BYTES;    // per stage: lse2[64], delta[64] of the streamed rows
+  uint8_t* sStat = sE1 + (DKDV ? 2 : 0) * TILE_BYTES;    // per stage: lse2[64], delta[64] of the streamed rows
   uint64_t* bars = (uint64_t*)(sStat + NST * 512);
   uint64_t *x_full = bars, *y_full = bars + 1, *y_empty = bars + 1 + NST, *t_full = bars + 1 + 2 * NST, *e_full = t_full + 1,
            *e_empty = t_full + 2, *acc_full = t_full + 3, *t_free = t_full + 4;
@@ -346,6 +364,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   const uint32_t tT0 = tmem_base, tT1 = tmem_base + 64, tA0 = tmem_base + 128, tA1 = tmem_base + 192;
+  const uint32_t tE = tmem_base + 128;                   // DQ only (no dV accumulator there): dS as bf16, 32 columns
 
   if (warp == 0) {
     if (lane == 0) {
@@ -408,8 +427,10 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
             umma_bf16(tA0, smem_desc(aE0 + kk * 32, 16, 1024), smem_desc(aY1 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
         }
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk)                    // dK += dS^T Q   |   dQ += dS K
-          umma_bf16(tA1, smem_desc(aE1 + kk * 32, 16, 1024), smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
+        for (int kk = 0; kk < 4; ++kk) {                  // dK += dS^T Q   |   dQ += dS K
+          if (DKDV) umma_bf16(tA1, smem_desc(aE1 + kk * 32, 16, 1024), smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
+          else umma_bf16_ts(tA1, tE + kk * 8, smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);   // dS from TMEM
+        }
         umma_commit(&y_empty[st]);
         umma_commit(e_empty);
       }
@@ -488,13 +509,21 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       TICK(2);
       if (t > 0) mbar_wait_many(e_empty, (uint32_t)(t - 1) & 1u, 27);        // ACC_{t-1} has finished reading E
       TICK(3);
+      if (DKDV) {
 #pragma unroll
-      for (int ch = 0; ch < CW / 8; ++ch) {
-        const uint32_t off = (uint32_t)(((cw0 / 8 + ch) ^ (r & 7)) << 4);
-        if (DKDV) sts128(e0row + off, wp[4 * ch], wp[4 * ch + 1], wp[4 * ch + 2], wp[4 * ch + 3]);
-        sts128(e1row + off, wd[4 * ch], wd[4 * ch + 1], wd[4 * ch + 2], wd[4 * ch + 3]);
+        for (int ch = 0; ch < CW / 8; ++ch) {
+          const uint32_t off = (uint32_t)(((cw0 / 8 + ch) ^ (r & 7)) << 4);
+          sts128(e0row + off, wp[4 * ch], wp[4 * ch + 1], wp[4 * ch + 2], wp[4 * ch + 3]);
+          sts128(e1row + off, wd[4 * ch], wd[4 * ch + 1], wd[4 * ch + 2], wd[4 * ch + 3]);
+        }
+        fence_async_smem();
+      } else {
+        // dQ kernel: dS goes to TENSOR MEMORY (the thread's lane, CW/2 packed columns) and is the A operand of
+        // dQ += dS K straight from there: no shared-memory round trip, no proxy fence
+        static_assert(CW == 32, "tcgen05.st x16 per thread");
+        tmem_st16(tE + lane_off + cw0 / 2, wd);
+        tmem_st_wait();
       }
-      fence_async_smem();
       tc_fence_before();
       mbar_arrive(e_full);
       TICK(4);
