@@ -289,8 +289,8 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
 // Two launches of ONE kernel template (deterministic, no atomics), both with this skeleton: two STATIONARY
 // 128-row tiles X0, X1 and a stream of 64-row tile pairs Y0, Y1 (2-stage TMA ring); per step
 //     T0 = X0 Y0^T,  T1 = X1 Y1^T            (M128 N64 K64, into TMEM)
-//     E0, E1 = elementwise(T0, T1)           (thread = TMEM lane = stationary row; bf16 into swizzled smem)
-//     ACC0 += E0 Y1,  ACC1 += E1 Y0          (M128 N64 K64, TMEM accumulators across all steps)
+//     E0, E1 = elementwise(T0, T1)           (thread = TMEM lane = stationary row; bf16 back into TMEM)
+//     ACC0 += E0 Y1,  ACC1 += E1 Y0          (M128 N64 K64, A operand from TMEM, accumulators in TMEM)
 //   DKDV (one CTA per 128-key block): X = K_j, V_j; Y = Q_i, dO_i over the query steps at or below the
 //        diagonal.  T0 = S^T, T1 = dP^T, E0 = P^T, E1 = dS^T; ACC0 = dV = P^T dO, ACC1 = dK = dS^T Q.
 //        lse and delta are indexed by the streamed (query) index: 2 x 256 B per step ride the same ring.
@@ -299,14 +299,14 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
 // with P = exp2(S c - lse log2e), dS = P o (dP - delta) / sqrt(dh); the probabilities are recomputed from the
 // stashed q, k and lse -- no parameter is involved, so this is not the checkpointed variant of P:282.
 // T_{t+1} is issued before ACC_t, so the tensor pipe computes the next scores while the 128 elementwise
-// threads work; two CTAs (96 KB smem, 256 TMEM columns each) share an SM.
+// threads work; two CTAs (98 KB smem, 256 TMEM columns each) share an SM.
 constexpr int BWD_EW = 2;                               // elementwise warpgroups: each thread owns 64/EW columns
 constexpr int BWD_THREADS = 64 + 128 * BWD_EW;
 constexpr uint32_t HALF_BYTES = 64 * 128;               // 64 rows x 64 bf16
-// ring depth: DKDV keeps both E tiles (P^T, dS^T) in shared memory and fits 2 stages in half an SM; DQ (dS in TMEM) takes 4
-__host__ __device__ constexpr int bwd_stages(bool dkdv) { return dkdv ? 2 : 4; }
+// ring depth of the streamed tiles (P^T / dS^T live in TMEM, so 4 stages fit in half an SM's shared memory)
+__host__ __device__ constexpr int bwd_stages(bool dkdv) { return dkdv ? 4 : 4; }
 __host__ __device__ constexpr uint32_t bwd_smem(bool dkdv) {
-  return 2 * TILE_BYTES + bwd_stages(dkdv) * (2 * HALF_BYTES + 512) + (dkdv ? 2u : 0u) * TILE_BYTES + 256;   // DQ: dS lives in TMEM
+  return 2 * TILE_BYTES + bwd_stages(dkdv) * (2 * HALF_BYTES + 512) + 256;   // P^T / dS^T live in TMEM
 }
 
 __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
@@ -326,9 +326,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   uint8_t* sX1 = sX0 + TILE_BYTES;
   uint8_t* sY = sX1 + TILE_BYTES;
   constexpr int NST = bwd_stages(DKDV);
-  uint8_t* sE1 = sY + NST * YST;
-  uint8_t* sE0 = sE1 + TILE_BYTES;                       // DKDV only
-  uint8_t* sStat = sE1 + (DKDV ? 2 : 0) * TILE_BYTES;    // per stage: lse2[64], delta[64] of the streamed rows
+  uint8_t* sStat = sY + NST * YST;                       // per stage: lse2[64], delta[64] of the streamed rows
   uint64_t* bars = (uint64_t*)(sStat + NST * 512);
   uint64_t *x_full = bars, *y_full = bars + 1, *y_empty = bars + 1 + NST, *t_full = bars + 1 + 2 * NST, *e_full = t_full + 1,
            *e_empty = t_full + 2, *acc_full = t_full + 3, *t_free = t_full + 4;
@@ -394,45 +392,57 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   } else if (warp == 1) {
     if (lane == 0) {
       constexpr uint32_t ID_T = idesc(128, 64, false, false), ID_ACC = idesc(128, 64, false, true);
-      const uint32_t aX0 = smem_u32(sX0), aX1 = smem_u32(sX1), aE0 = smem_u32(sE0), aE1 = smem_u32(sE1);
-      auto issue_t = [&](int t) {
+      const uint32_t aX0 = smem_u32(sX0), aX1 = smem_u32(sX1);
+      auto issue_t0 = [&](int t) {
         const int st = t % NST;
         mbar_wait(&y_full[st], (uint32_t)(t / NST) & 1u, 22);
         tc_fence_after();
-        const uint32_t aY0 = smem_u32(sY + st * YST), aY1 = aY0 + HALF_BYTES;
+        const uint32_t aY0 = smem_u32(sY + st * YST);
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)
           umma_bf16(tT0, smem_desc(aX0 + kk * 32, 16, 1024), smem_desc(aY0 + kk * 32, 16, 1024), ID_T, kk > 0 ? 1u : 0u);
+      };
+      auto issue_t1 = [&](int t) {                        // after issue_t0(t): the stage is known to have landed
+        const uint32_t aY1 = smem_u32(sY + (t % NST) * YST) + HALF_BYTES;
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)
           umma_bf16(tT1, smem_desc(aX1 + kk * 32, 16, 1024), smem_desc(aY1 + kk * 32, 16, 1024), ID_T, kk > 0 ? 1u : 0u);
         umma_commit(t_full);
       };
       mbar_wait(x_full, 0, 23);
-      issue_t(0);
+      issue_t0(0);
+      issue_t1(0);
       for (int t = 0; t < n_steps; ++t) {
         if (t + 1 < n_steps) {                            // T_t sits in the elementwise threads' registers: the next
           mbar_wait(t_free, (uint32_t)t & 1u, 29);         // score-type MMAs run WHILE they do exp2 / pack
           tc_fence_after();
-          issue_t(t + 1);
+          issue_t0(t + 1);
+          if (!DKDV) issue_t1(t + 1);
         }
-        mbar_wait(e_full, (uint32_t)t & 1u, 24);          // E_t is in shared memory
+        mbar_wait(e_full, (uint32_t)t & 1u, 24);          // E_t is in tensor memory
         tc_fence_after();
         const int st = t % NST;
         const uint32_t aY0 = smem_u32(sY + st * YST), aY1 = aY0 + HALF_BYTES;
         const uint32_t acc = t > 0 ? 1u : 0u;
         if (DKDV) {
+          // P^T and dS^T (bf16) sit in T1's 64 columns: warpgroup g wrote its 32 queries of P^T at +32 g and of dS^T
+          // at +32 g + 16; one K = 16 step of the A operand is 8 columns
 #pragma unroll
           for (int kk = 0; kk < 4; ++kk)                  // dV += P^T dO
-            umma_bf16(tA0, smem_desc(aE0 + kk * 32, 16, 1024), smem_desc(aY1 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
-        }
+            umma_bf16_ts(tA0, tT1 + 32 * (kk >> 1) + 8 * (kk & 1), smem_desc(aY1 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
 #pragma unroll
-        for (int kk = 0; kk < 4; ++kk) {                  // dK += dS^T Q   |   dQ += dS K
-          if (DKDV) umma_bf16(tA1, smem_desc(aE1 + kk * 32, 16, 1024), smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
-          else umma_bf16_ts(tA1, tE + kk * 8, smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);   // dS from TMEM
+          for (int kk = 0; kk < 4; ++kk)                  // dK += dS^T Q
+            umma_bf16_ts(tA1, tT1 + 32 * (kk >> 1) + 16 + 8 * (kk & 1), smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
+        } else {
+#pragma unroll
+          for (int kk = 0; kk < 4; ++kk)                  // dQ += dS K, dS from its own TMEM columns
+            umma_bf16_ts(tA1, tE + kk * 8, smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
         }
         umma_commit(&y_empty[st]);
         umma_commit(e_empty);
+        // dK/dV: T1_{t+1} overwrites the columns P^T / dS^T were read from, so it is issued AFTER the accumulate
+        // MMAs of step t (the tensor pipe executes one thread's MMAs in order)
+        if (DKDV && t + 1 < n_steps) issue_t1(t + 1);
       }
       umma_commit(acc_full);
     }
@@ -452,8 +462,6 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       my_lse2 = lse[((size_t)b * H + h) * T + x0 + r];
       my_delta = delta[((size_t)b * H + h) * T + x0 + r];
     }
-    uint8_t* e0row = sE0 + r * 128;
-    uint8_t* e1row = sE1 + r * 128;
 #ifdef PACI_ATTN_TIMING
     long long tk[6] = {0, 0, 0, 0, 0, 0}, tprev = clock64(), tnow;
 #define TICK(i) do { tnow = clock64(); tk[i] += tnow - tprev; tprev = tnow; } while (0)
@@ -509,21 +517,17 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       TICK(2);
       if (t > 0) mbar_wait_many(e_empty, (uint32_t)(t - 1) & 1u, 27);        // ACC_{t-1} has finished reading E
       TICK(3);
+      // P^T / dS^T go to TENSOR MEMORY (the thread's lane, CW/2 packed columns each) and are the A operands of the
+      // accumulate MMAs straight from there: no shared-memory round trip, no proxy fence.  dK/dV: they overwrite
+      // this thread's own 32 columns of T1 (already in its registers); dQ: dS has columns of its own.
+      static_assert(CW == 32, "tcgen05.st x16 per thread");
       if (DKDV) {
-#pragma unroll
-        for (int ch = 0; ch < CW / 8; ++ch) {
-          const uint32_t off = (uint32_t)(((cw0 / 8 + ch) ^ (r & 7)) << 4);
-          sts128(e0row + off, wp[4 * ch], wp[4 * ch + 1], wp[4 * ch + 2], wp[4 * ch + 3]);
-          sts128(e1row + off, wd[4 * ch], wd[4 * ch + 1], wd[4 * ch + 2], wd[4 * ch + 3]);
-        }
-        fence_async_smem();
+        tmem_st16(tT1 + lane_off + cw0, wp);
+        tmem_st16(tT1 + lane_off + cw0 + 16, wd);
       } else {
-        // dQ kernel: dS goes to TENSOR MEMORY (the thread's lane, CW/2 packed columns) and is the A operand of
-        // dQ += dS K straight from there: no shared-memory round trip, no proxy fence
-        static_assert(CW == 32, "tcgen05.st x16 per thread");
         tmem_st16(tE + lane_off + cw0 / 2, wd);
-        tmem_st_wait();
       }
+      tmem_st_wait();
       tc_fence_before();
       mbar_arrive(e_full);
       TICK(4);
