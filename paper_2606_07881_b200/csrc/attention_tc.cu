@@ -1,7 +1,7 @@
 // attention_tc.cu -- fused causal attention on the 5th-generation tensor cores (tcgen05 + TMEM + TMA),
 // bf16, head dim 64, T a multiple of 128 (rows a4, a17 of SURVEY.md 8(a)).
 //
-// Forward.  One CTA = 128 query rows of one (batch, head); key blocks of 128; two CTAs per SM (115 KB of
+// Forward.  One CTA = 128 query rows of one (batch, head); key blocks of 128; two CTAs per SM (82 KB of
 // shared memory and 256 TMEM columns each), so one CTA's softmax overlaps the other CTA's MMAs.
 //   warp 0     TMA producer: Q once, then K_j / V_j through 2-stage rings (one 2D tensor map over the packed
 //              qkv tensor [mu*T, 3D], box 64 columns x 128 rows, 128-byte swizzle)
@@ -9,8 +9,8 @@
 //              O += P_j V_j (M128 N64 K128) into columns 128..191; S_{j+1} is issued before P_j V_j so the
 //              tensor pipe always has the next scores ready
 //   warps 2-5  softmax: thread = query row (TMEM lane).  One pass over S: tcgen05.ld 128 columns, row max,
-//              p = exp2(s * c - m_ref), row sum, P as bf16 into 128B-swizzled shared memory (the A operand of
-//              P V).  O stays in TMEM across key blocks (accumulate = 1) and is rescaled only when the running
+//              p = exp2(s * c - m_ref), row sum, P as packed bf16 back into TMEM (tcgen05.st), the A operand of
+//              P V (no shared-memory round trip).  O stays in TMEM across key blocks (accumulate = 1) and is rescaled only when the running
 //              max has grown by more than 2^8 since the reference max m_ref was taken ("lazy rescale"): the
 //              final O / l and lse = m_ref + log2 l do not depend on which reference was used.
 // qkv is packed [mu, T, 3D]: q | k | v, head h at columns h*64 .. h*64+63 (R17).
@@ -89,7 +89,7 @@ __host__ __device__ constexpr uint32_t idesc(int M, int N, bool a_mn, bool b_mn)
 // ============================================================================== forward
 constexpr int FWD_THREADS = 192;
 constexpr uint32_t TILE_BYTES = 128 * 128;              // 128 rows x 64 bf16
-constexpr uint32_t FWD_SMEM = TILE_BYTES * (1 + 2 + 2) + 2 * TILE_BYTES + 256;   // Q, K[2], V[2], P (2 tiles), barriers
+constexpr uint32_t FWD_SMEM = TILE_BYTES * (1 + 2 + 2) + 256;   // Q, K[2], V[2], barriers (P lives in TMEM)
 
 __global__ void __launch_bounds__(FWD_THREADS, 2)
 attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* __restrict__ o,
@@ -98,8 +98,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
   uint8_t* sQ = smem;
   uint8_t* sK = sQ + TILE_BYTES;
   uint8_t* sV = sK + 2 * TILE_BYTES;
-  uint8_t* sP = sV + 2 * TILE_BYTES;
-  uint64_t* bars = (uint64_t*)(sP + 2 * TILE_BYTES);
+  uint64_t* bars = (uint64_t*)(sV + 2 * TILE_BYTES);
   uint64_t *q_full = bars, *k_full = bars + 1, *v_full = bars + 3, *k_empty = bars + 5, *v_empty = bars + 7,
            *s_full = bars + 9, *p_full = bars + 10, *o_full = bars + 11, *s_free = bars + 12;
   uint32_t* tmem_slot = (uint32_t*)(bars + 13);
@@ -129,7 +128,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
-  const uint32_t tS = tmem_base, tO = tmem_base + 128;
+  const uint32_t tS = tmem_base, tO = tmem_base + 128, tP = tmem_base + 192;   // P: 128 keys as bf16 = 64 columns
 
   if (warp == 0) {
     if (lane == 0) {
@@ -151,7 +150,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
   } else if (warp == 1) {
     if (lane == 0) {
       constexpr uint32_t ID_QK = idesc(128, 128, false, false), ID_PV = idesc(128, 64, false, true);
-      const uint32_t aQ = smem_u32(sQ), aP = smem_u32(sP);
+      const uint32_t aQ = smem_u32(sQ);
       auto issue_qk = [&](int j) {
         const int st = j & 1;
         mbar_wait(&k_full[st], (uint32_t)(j >> 1) & 1u, 13);
@@ -179,8 +178,8 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
         const uint32_t aV = smem_u32(sV + st * TILE_BYTES);
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks)                    // 8 x 16 keys
-          umma_bf16(tO, smem_desc(aP + (ks >> 2) * TILE_BYTES + (ks & 3) * 32, 16, 1024),
-                    smem_desc(aV + (ks >> 2) * 8192 + (ks & 3) * 2048, 8192, 1024), ID_PV, (j > 0 || ks > 0) ? 1u : 0u);
+          umma_bf16_ts(tO, tP + ks * 8, smem_desc(aV + (ks >> 2) * 8192 + (ks & 3) * 2048, 8192, 1024), ID_PV,
+                       (j > 0 || ks > 0) ? 1u : 0u);                 // P from tensor memory: 8 columns per K = 16
         umma_commit(&v_empty[st]);
         umma_commit(o_full);
       }
@@ -190,7 +189,6 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
     const float c = rsqrtf((float)DH) * LOG2E;
     float m_ref = -INFINITY, l = 0.f;
-    uint8_t* prow = sP + r * 128;
     for (int j = 0; j < n_kb; ++j) {
       mbar_wait_many(s_full, (uint32_t)j & 1u, 17);
       tc_fence_after();
@@ -239,20 +237,21 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
       if (j > 0) { mbar_wait_many(o_full, (uint32_t)(j - 1) & 1u, 30); tc_fence_after(); }
       float sum4[4] = {0.f, 0.f, 0.f, 0.f};
       const float neg_m = -m_ref;
+      // P goes registers -> TENSOR MEMORY (packed bf16, this thread's lane) and is the A operand of P V from there
 #pragma unroll
-      for (int ch = 0; ch < 16; ++ch) {                   // 16 chunks of 8 keys = 16 bytes of bf16
-        uint32_t w[4];
+      for (int half = 0; half < 2; ++half) {
+        uint32_t w[32];
 #pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          const float p0 = ex2(fmaf(__uint_as_float(s[ch * 8 + 2 * t]), c, neg_m));       // exp2(-inf) = 0: masked
-          const float p1 = ex2(fmaf(__uint_as_float(s[ch * 8 + 2 * t + 1]), c, neg_m));
-          sum4[t] += p0 + p1;
+        for (int t = 0; t < 32; ++t) {
+          const float p0 = ex2(fmaf(__uint_as_float(s[half * 64 + 2 * t]), c, neg_m));       // exp2(-inf) = 0: masked
+          const float p1 = ex2(fmaf(__uint_as_float(s[half * 64 + 2 * t + 1]), c, neg_m));
+          sum4[t & 3] += p0 + p1;
           w[t] = pack_bf16x2(p0, p1);
         }
-        sts128(prow + (ch >> 3) * TILE_BYTES + (((ch & 7) ^ (r & 7)) << 4), w[0], w[1], w[2], w[3]);
+        tmem_st32(tP + lane_off + half * 32, w);
       }
       l += (sum4[0] + sum4[1]) + (sum4[2] + sum4[3]);
-      fence_async_smem();                                 // P visible to the tensor core's async proxy
+      tmem_st_wait();
       tc_fence_before();
       mbar_arrive(p_full);
     }
