@@ -14,6 +14,7 @@
 //              max has grown by more than 2^8 since the reference max m_ref was taken ("lazy rescale"): the
 //              final O / l and lse = m_ref + log2 l do not depend on which reference was used.
 // qkv is packed [mu, T, 3D]: q | k | v, head h at columns h*64 .. h*64+63 (R17).
+#include <cstdlib>
 #include <type_traits>
 
 #include "tc_ptx.cuh"
@@ -313,12 +314,17 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
                ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+// PERSISTENT: the grid is two CTAs per SM; each CTA takes (tile, head, batch) items off a global counter (heaviest
+// tiles first), so barrier setup, the TMEM allocation and the descriptor fetches are paid once per CTA, the
+// stationary tiles of the next item load while the last step of the current one is being reduced, and the tail of
+// the launch is balanced dynamically.  `g` counts streamed steps over the CTA's whole life: the ring and the
+// per-step barriers are indexed by it; x_full / acc_full / acc_empty / x_empty complete once per item.
 template <bool DKDV, int EW>
 __global__ void __launch_bounds__(64 + 128 * EW, 2)
 attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constant__ CUtensorMap mX1,
-                   const __grid_constant__ CUtensorMap mY0, const __grid_constant__ CUtensorMap mY1, int T, int H,
+                   const __grid_constant__ CUtensorMap mY0, const __grid_constant__ CUtensorMap mY1, int T, int H, int mu,
                    const float* __restrict__ lse, const float* __restrict__ delta, bf16* __restrict__ dqkv,
-                   float* __restrict__ Gbias) {
+                   float* __restrict__ Gbias, int* __restrict__ work_counter) {
   extern __shared__ __align__(1024) uint8_t smem[];
   constexpr uint32_t YST = 2 * HALF_BYTES;               // one ring stage: Y0, Y1 (1024-byte aligned tiles)
   uint8_t* sX0 = smem;
@@ -328,28 +334,38 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   uint8_t* sStat = sY + NST * YST;                       // per stage: lse2[64], delta[64] of the streamed rows
   uint64_t* bars = (uint64_t*)(sStat + NST * 512);
   uint64_t *x_full = bars, *y_full = bars + 1, *y_empty = bars + 1 + NST, *t_full = bars + 1 + 2 * NST, *e_full = t_full + 1,
-           *e_empty = t_full + 2, *acc_full = t_full + 3, *t_free = t_full + 4;
-  uint32_t* tmem_slot = (uint32_t*)(t_full + 5);
+           *e_empty = t_full + 2, *acc_full = t_full + 3, *t_free = t_full + 4, *x_empty = t_full + 5, *acc_empty = t_full + 6,
+           *item_full = t_full + 7;                      // [2]
+  uint32_t* tmem_slot = (uint32_t*)(t_full + 9);
+  volatile int* item_slot = (volatile int*)(tmem_slot + 1);   // [2]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int D = H * DH;
   const int nt = T / 128;
-  const int per = H * (int)(gridDim.x / (nt * H));       // H * mu
-  const int rank = (int)blockIdx.x / per;                // heaviest tiles first
-  const int tile = DKDV ? rank : nt - 1 - rank;
-  const int rem = (int)blockIdx.x % per;
-  const int h = rem % H, b = rem / H;
-  const int x0 = tile * 128;                             // first stationary row (key for DKDV, query for DQ)
-  const int c_begin = DKDV ? x0 : 0;                     // streamed rows [c_begin, c_end), 64 per step
-  const int c_end = DKDV ? T : x0 + 128;
-  const int n_steps = (c_end - c_begin) / 64;
-  const int row0 = b * T;
+  const int per = H * mu;
+  const int n_items = nt * per;
+  // item -> (first stationary row, head, first token row of the batch element, streamed range)
+  struct Item { int x0, h, row0, c_begin, n_steps, bh; };
+  auto decode = [&](int item) {
+    Item it;
+    const int rank = item / per, rem = item % per;       // heaviest tiles first
+    const int tile = DKDV ? rank : nt - 1 - rank;
+    it.h = rem % H;
+    const int b = rem / H;
+    it.x0 = tile * 128;                                  // first stationary row (key for DKDV, query for DQ)
+    it.c_begin = DKDV ? it.x0 : 0;                       // streamed rows [c_begin, c_end), 64 per step
+    it.n_steps = ((DKDV ? T : it.x0 + 128) - it.c_begin) / 64;
+    it.row0 = b * T;
+    it.bh = b * H + it.h;
+    return it;
+  };
 
   if ((smem_u32(smem) & 1023u) != 0) __trap();
   if (threadIdx.x == 0) {
     mbar_init(x_full, 1);
     for (int i = 0; i < NST; ++i) { mbar_init(&y_full[i], 1); mbar_init(&y_empty[i], 1); }
     mbar_init(t_full, 1); mbar_init(e_full, 128 * EW); mbar_init(e_empty, 1); mbar_init(acc_full, 1); mbar_init(t_free, 128 * EW);
+    mbar_init(x_empty, 1); mbar_init(acc_empty, 128 * EW); mbar_init(&item_full[0], 1); mbar_init(&item_full[1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 1) {
@@ -365,26 +381,37 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
 
   if (warp == 0) {
     if (lane == 0) {
-      // column of each operand inside its tensor: qkv = [q | k | v], dO = [D]
-      const int cx0 = DKDV ? D + h * DH : h * DH;        // K_j | Q_i
-      const int cx1 = DKDV ? 2 * D + h * DH : h * DH;    // V_j | dO_i
-      const int cy0 = DKDV ? h * DH : D + h * DH;        // Q   | K
-      const int cy1 = DKDV ? h * DH : 2 * D + h * DH;    // dO  | V
-      mbar_expect_tx(x_full, 2 * TILE_BYTES);
-      tma_load_2d(sX0, &mX0, x_full, cx0, row0 + x0);
-      tma_load_2d(sX1, &mX1, x_full, cx1, row0 + x0);
-      const float* lrow = lse + ((size_t)b * H + h) * T;
-      const float* drow = delta + ((size_t)b * H + h) * T;
-      for (int t = 0; t < n_steps; ++t) {
-        const int st = t % NST, c0 = c_begin + t * 64;
-        mbar_wait(&y_empty[st], ((uint32_t)(t / NST) & 1u) ^ 1u, 21);
-        uint8_t* y = sY + st * YST;
-        mbar_expect_tx(&y_full[st], 2 * HALF_BYTES + (DKDV ? 512u : 0u));
-        tma_load_2d(y, &mY0, &y_full[st], cy0, row0 + c0);
-        tma_load_2d(y + HALF_BYTES, &mY1, &y_full[st], cy1, row0 + c0);
-        if (DKDV) {
-          bulk_load_1d(sStat + st * 512, lrow + c0, 256, &y_full[st]);
-          bulk_load_1d(sStat + st * 512 + 256, drow + c0, 256, &y_full[st]);
+      uint32_t g = 0;
+      for (uint32_t k = 0;; ++k) {
+        // the slot of item k-2 is free: every consumer copied it before item k-1's stationary tiles could be
+        // requested (x_empty of k-2), which happened before this point
+        const int item = atomicAdd(work_counter, 1);
+        item_slot[k & 1] = item;
+        mbar_arrive(&item_full[k & 1]);                  // release: the slot write is visible to the waiters
+        if (item >= n_items) break;
+        const Item it = decode(item);
+        // column of each operand inside its tensor: qkv = [q | k | v], dO = [D]
+        const int cx0 = DKDV ? D + it.h * DH : it.h * DH;        // K_j | Q_i
+        const int cx1 = DKDV ? 2 * D + it.h * DH : it.h * DH;    // V_j | dO_i
+        const int cy0 = DKDV ? it.h * DH : D + it.h * DH;        // Q   | K
+        const int cy1 = DKDV ? it.h * DH : 2 * D + it.h * DH;    // dO  | V
+        mbar_wait(x_empty, (k & 1u) ^ 1u, 20);           // the previous item's score MMAs have read X
+        mbar_expect_tx(x_full, 2 * TILE_BYTES);
+        tma_load_2d(sX0, &mX0, x_full, cx0, it.row0 + it.x0);
+        tma_load_2d(sX1, &mX1, x_full, cx1, it.row0 + it.x0);
+        const float* lrow = lse + (size_t)it.bh * T;
+        const float* drow = delta + (size_t)it.bh * T;
+        for (int t = 0; t < it.n_steps; ++t, ++g) {
+          const int st = g % NST, c0 = it.c_begin + t * 64;
+          mbar_wait(&y_empty[st], ((g / NST) & 1u) ^ 1u, 21);
+          uint8_t* y = sY + st * YST;
+          mbar_expect_tx(&y_full[st], 2 * HALF_BYTES + (DKDV ? 512u : 0u));
+          tma_load_2d(y, &mY0, &y_full[st], cy0, it.row0 + c0);
+          tma_load_2d(y + HALF_BYTES, &mY1, &y_full[st], cy1, it.row0 + c0);
+          if (DKDV) {
+            bulk_load_1d(sStat + st * 512, lrow + c0, 256, &y_full[st]);
+            bulk_load_1d(sStat + st * 512 + 256, drow + c0, 256, &y_full[st]);
+          }
         }
       }
     }
@@ -392,58 +419,80 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
     if (lane == 0) {
       constexpr uint32_t ID_T = idesc(128, 64, false, false), ID_ACC = idesc(128, 64, false, true);
       const uint32_t aX0 = smem_u32(sX0), aX1 = smem_u32(sX1);
-      auto issue_t0 = [&](int t) {
-        const int st = t % NST;
-        mbar_wait(&y_full[st], (uint32_t)(t / NST) & 1u, 22);
+      auto issue_t0 = [&](uint32_t gs) {
+        const int st = gs % NST;
+        mbar_wait(&y_full[st], (gs / NST) & 1u, 22);
         tc_fence_after();
         const uint32_t aY0 = smem_u32(sY + st * YST);
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)
           umma_bf16(tT0, smem_desc(aX0 + kk * 32, 16, 1024), smem_desc(aY0 + kk * 32, 16, 1024), ID_T, kk > 0 ? 1u : 0u);
       };
-      auto issue_t1 = [&](int t) {                        // after issue_t0(t): the stage is known to have landed
-        const uint32_t aY1 = smem_u32(sY + (t % NST) * YST) + HALF_BYTES;
+      auto issue_t1 = [&](uint32_t gs) {                  // after issue_t0(gs): the stage is known to have landed
+        const uint32_t aY1 = smem_u32(sY + (gs % NST) * YST) + HALF_BYTES;
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)
           umma_bf16(tT1, smem_desc(aX1 + kk * 32, 16, 1024), smem_desc(aY1 + kk * 32, 16, 1024), ID_T, kk > 0 ? 1u : 0u);
         umma_commit(t_full);
       };
-      mbar_wait(x_full, 0, 23);
-      issue_t0(0);
-      issue_t1(0);
-      for (int t = 0; t < n_steps; ++t) {
-        if (t + 1 < n_steps) {                            // T_t sits in the elementwise threads' registers: the next
-          mbar_wait(t_free, (uint32_t)t & 1u, 29);         // score-type MMAs run WHILE they do exp2 / pack
+      uint32_t g = 0;
+      for (uint32_t k = 0;; ++k) {
+        mbar_wait(&item_full[k & 1], (k >> 1) & 1u, 19);
+        const int item = item_slot[k & 1];
+        if (item >= n_items) break;
+        const int n_steps = decode(item).n_steps;
+        mbar_wait(x_full, k & 1u, 23);
+        if (g > 0) {                                      // the previous item's last T0 / T1 are in registers
+          mbar_wait(t_free, (g - 1) & 1u, 29);
           tc_fence_after();
-          issue_t0(t + 1);
-          if (!DKDV) issue_t1(t + 1);
         }
-        mbar_wait(e_full, (uint32_t)t & 1u, 24);          // E_t is in tensor memory
-        tc_fence_after();
-        const int st = t % NST;
-        const uint32_t aY0 = smem_u32(sY + st * YST), aY1 = aY0 + HALF_BYTES;
-        const uint32_t acc = t > 0 ? 1u : 0u;
-        if (DKDV) {
-          // P^T and dS^T (bf16) sit in T1's 64 columns: warpgroup g wrote its 32 queries of P^T at +32 g and of dS^T
-          // at +32 g + 16; one K = 16 step of the A operand is 8 columns
-#pragma unroll
-          for (int kk = 0; kk < 4; ++kk)                  // dV += P^T dO
-            umma_bf16_ts(tA0, tT1 + 32 * (kk >> 1) + 8 * (kk & 1), smem_desc(aY1 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
-#pragma unroll
-          for (int kk = 0; kk < 4; ++kk)                  // dK += dS^T Q
-            umma_bf16_ts(tA1, tT1 + 32 * (kk >> 1) + 16 + 8 * (kk & 1), smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
-        } else {
-#pragma unroll
-          for (int kk = 0; kk < 4; ++kk)                  // dQ += dS K, dS from its own TMEM columns
-            umma_bf16_ts(tA1, tE + kk * 8, smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
+        issue_t0(g);
+        issue_t1(g);                                      // (dK/dV) in order behind the previous item's last accumulate MMAs
+        if (k > 0) {                                      // the previous item's accumulators have been read out
+          mbar_wait(acc_empty, (k - 1) & 1u, 18);
+          tc_fence_after();
         }
-        umma_commit(&y_empty[st]);
-        umma_commit(e_empty);
-        // dK/dV: T1_{t+1} overwrites the columns P^T / dS^T were read from, so it is issued AFTER the accumulate
-        // MMAs of step t (the tensor pipe executes one thread's MMAs in order)
-        if (DKDV && t + 1 < n_steps) issue_t1(t + 1);
+        for (int t = 0; t < n_steps; ++t, ++g) {
+          const bool more = t + 1 < n_steps;
+          if (more) {                                     // T_t sits in the elementwise threads' registers: the next
+            mbar_wait(t_free, g & 1u, 29);                // score-type MMAs run WHILE they do exp2 / pack
+            tc_fence_after();
+            issue_t0(g + 1);
+            if (!DKDV) {
+              issue_t1(g + 1);
+              if (t + 2 == n_steps) umma_commit(x_empty); // X is not read again: the next item's may load
+            }
+          }
+          mbar_wait(e_full, g & 1u, 24);                  // E_t is in tensor memory
+          tc_fence_after();
+          const int st = g % NST;
+          const uint32_t aY0 = smem_u32(sY + st * YST), aY1 = aY0 + HALF_BYTES;
+          const uint32_t acc = t > 0 ? 1u : 0u;
+          if (DKDV) {
+            // P^T and dS^T (bf16) sit in T1's 64 columns: warpgroup g wrote its 32 queries of P^T at +32 g and of dS^T
+            // at +32 g + 16; one K = 16 step of the A operand is 8 columns
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk)                // dV += P^T dO
+              umma_bf16_ts(tA0, tT1 + 32 * (kk >> 1) + 8 * (kk & 1), smem_desc(aY1 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk)                // dK += dS^T Q
+              umma_bf16_ts(tA1, tT1 + 32 * (kk >> 1) + 16 + 8 * (kk & 1), smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
+          } else {
+#pragma unroll
+            for (int kk = 0; kk < 4; ++kk)                // dQ += dS K, dS from its own TMEM columns
+              umma_bf16_ts(tA1, tE + kk * 8, smem_desc(aY0 + kk * 2048, 8192, 1024), ID_ACC, (acc | (kk > 0)) ? 1u : 0u);
+          }
+          umma_commit(&y_empty[st]);
+          umma_commit(e_empty);
+          // dK/dV: T1_{t+1} overwrites the columns P^T / dS^T were read from, so it is issued AFTER the accumulate
+          // MMAs of step t (the tensor pipe executes one thread's MMAs in order)
+          if (DKDV && more) {
+            issue_t1(g + 1);
+            if (t + 2 == n_steps) umma_commit(x_empty);
+          }
+        }
+        umma_commit(acc_full);
       }
-      umma_commit(acc_full);
     }
   } else {
     // EW warpgroups of 4 warps: warp w owns TMEM lanes 32 (w % 4) .., warpgroup g = (w - 2) / 4 owns columns
@@ -456,90 +505,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
     const int cw0 = wg * CW;
     const uint32_t lane_off = (uint32_t)((warp & 3) * 32) << 16;
     const float c = rsqrtf((float)DH) * LOG2E;
-    float my_lse2 = 0.f, my_delta = 0.f;
-    if (!DKDV) {
-      my_lse2 = lse[((size_t)b * H + h) * T + x0 + r];
-      my_delta = delta[((size_t)b * H + h) * T + x0 + r];
-    }
-#ifdef PACI_ATTN_TIMING
-    long long tk[6] = {0, 0, 0, 0, 0, 0}, tprev = clock64(), tnow;
-#define TICK(i) do { tnow = clock64(); tk[i] += tnow - tprev; tprev = tnow; } while (0)
-#else
-#define TICK(i) do {} while (0)
-#endif
-    for (int t = 0; t < n_steps; ++t) {
-      const int st = t % NST, c0 = c_begin + t * 64;
-      mbar_wait_many(t_full, (uint32_t)t & 1u, 25);
-      tc_fence_after();
-      TICK(0);
-      uint32_t s[CW], dp[CW];
-      tmem_ld_cols_nowait<CW>(tT0 + lane_off + cw0, s);
-      tmem_ld_cols_nowait<CW>(tT1 + lane_off + cw0, dp);
-      tmem_ld_wait();
-      tc_fence_before();
-      mbar_arrive(t_free);                                // T0 / T1 may be overwritten by step t+1's MMAs
-      TICK(1);
-      const float4* pl = reinterpret_cast<const float4*>(sStat + st * 512) + cw0 / 4;   // lse2 of the step's 64 queries
-      const float4* pd = pl + 16;                                                        // delta
-      if (DKDV) mbar_wait_many(&y_full[st], (uint32_t)(t / NST) & 1u, 26);   // the step's lse / delta have landed
-      // causal keep: query >= key.  DKDV: query = c0 + col, key = x0 + r.  DQ: query = x0 + r, key = c0 + col.
-      // Only the two diagonal steps need the mask; `rel` is the diagonal's column inside this thread's slice.
-      const bool diag = DKDV ? (c0 < x0 + 128) : (c0 + 63 > x0);
-      const int rel = x0 + r - c0 - cw0;
-      uint32_t wp[CW / 2], wd[CW / 2];
-      auto body = [&](auto masked) {
-#pragma unroll
-        for (int k4 = 0; k4 < CW / 4; ++k4) {
-          float l2[4] = {my_lse2, my_lse2, my_lse2, my_lse2}, dl[4] = {my_delta, my_delta, my_delta, my_delta};
-          if (DKDV) {
-            const float4 a4 = pl[k4], d4 = pd[k4];
-            l2[0] = a4.x; l2[1] = a4.y; l2[2] = a4.z; l2[3] = a4.w;
-            dl[0] = d4.x; dl[1] = d4.y; dl[2] = d4.z; dl[3] = d4.w;
-          }
-          float pv[4], dv[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int i = 4 * k4 + e;
-            float pr = ex2(fmaf(__uint_as_float(s[i]), c, -l2[e]));
-            if (decltype(masked)::value) {
-              const bool keep = DKDV ? (i >= rel) : (i <= rel);
-              pr = keep ? pr : 0.f;
-            }
-            pv[e] = pr;
-            dv[e] = pr * (__uint_as_float(dp[i]) - dl[e]);
-          }
-          wp[2 * k4] = pack_bf16x2(pv[0], pv[1]); wp[2 * k4 + 1] = pack_bf16x2(pv[2], pv[3]);
-          wd[2 * k4] = pack_bf16x2(dv[0], dv[1]); wd[2 * k4 + 1] = pack_bf16x2(dv[2], dv[3]);
-        }
-      };
-      if (diag) body(std::true_type{}); else body(std::false_type{});
-      TICK(2);
-      if (t > 0) mbar_wait_many(e_empty, (uint32_t)(t - 1) & 1u, 27);        // ACC_{t-1} has finished reading E
-      TICK(3);
-      // P^T / dS^T go to TENSOR MEMORY (the thread's lane, CW/2 packed columns each) and are the A operands of the
-      // accumulate MMAs straight from there: no shared-memory round trip, no proxy fence.  dK/dV: they overwrite
-      // this thread's own 32 columns of T1 (already in its registers); dQ: dS has columns of its own.
-      static_assert(CW == 32, "tcgen05.st x16 per thread");
-      if (DKDV) {
-        tmem_st16(tT1 + lane_off + cw0, wp);
-        tmem_st16(tT1 + lane_off + cw0 + 16, wd);
-      } else {
-        tmem_st16(tE + lane_off + cw0 / 2, wd);
-      }
-      tmem_st_wait();
-      tc_fence_before();
-      mbar_arrive(e_full);
-      TICK(4);
-    }
-#ifdef PACI_ATTN_TIMING
-    if (threadIdx.x == 64 && (blockIdx.x == 0 || blockIdx.x == 300 || blockIdx.x == 900))
-      printf("bwd dkdv=%d blk %d steps %d: wait_t %lld ldtm %lld compute %lld wait_e %lld sts+fence %lld (cycles per step)\n", (int)DKDV,
-             (int)blockIdx.x, n_steps, tk[0] / n_steps, tk[1] / n_steps, tk[2] / n_steps, tk[3] / n_steps, tk[4] / n_steps);
-#endif
-    // epilogue: accumulators -> bf16 rows of dqkv, 32-column chunks dealt round-robin to the warpgroups
-    mbar_wait_many(acc_full, 0, 28);
-    tc_fence_after();
-    bf16* orow = dqkv + ((size_t)row0 + x0 + r) * 3 * D + h * DH;
+    const float inv_sqrt = rsqrtf((float)DH);
     // Gbias (fp32 [3D], may be NULL): the bias gradient of the QKV projection = column sums of dqkv over all
     // tokens (row a15), taken here from the ROUNDED values being stored: one warp-shuffle reduction over the
     // warp's 32 rows per column, then one atomic per column per warp -- no separate pass over dqkv.
@@ -568,16 +534,93 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
         }
       }
     };
-    const float inv_sqrt = rsqrtf((float)DH);
-    constexpr int N_CHUNKS = DKDV ? 4 : 2;                // DKDV: dV lo, dV hi, dK lo, dK hi.  DQ: dQ lo, dQ hi
-    for (int k = wg; k < N_CHUNKS; k += EW) {             // warp-uniform
-      if (DKDV) {
-        const int col = (k < 2 ? 2 * D : D) + (k & 1) * 32;
-        store_chunk((k < 2 ? tA0 : tA1) + (k & 1) * 32, orow + col, k < 2 ? 1.f : inv_sqrt,
-                    Gbias != nullptr ? Gbias + h * DH + col : nullptr);
-      } else {
-        store_chunk(tA1 + k * 32, orow + k * 32, inv_sqrt, Gbias != nullptr ? Gbias + h * DH + k * 32 : nullptr);
+    uint32_t g = 0;
+    for (uint32_t k = 0;; ++k) {
+      mbar_wait_many(&item_full[k & 1], (k >> 1) & 1u, 17);
+      const int item = item_slot[k & 1];
+      if (item >= n_items) break;
+      const Item it = decode(item);
+      const int x0 = it.x0;
+      float my_lse2 = 0.f, my_delta = 0.f;
+      if (!DKDV) {
+        my_lse2 = lse[(size_t)it.bh * T + x0 + r];
+        my_delta = delta[(size_t)it.bh * T + x0 + r];
       }
+      for (int t = 0; t < it.n_steps; ++t, ++g) {
+        const int st = g % NST, c0 = it.c_begin + t * 64;
+        mbar_wait_many(t_full, g & 1u, 25);
+        tc_fence_after();
+        uint32_t s[CW], dp[CW];
+        tmem_ld_cols_nowait<CW>(tT0 + lane_off + cw0, s);
+        tmem_ld_cols_nowait<CW>(tT1 + lane_off + cw0, dp);
+        tmem_ld_wait();
+        tc_fence_before();
+        mbar_arrive(t_free);                              // T0 / T1 may be overwritten by the next step's MMAs
+        const float4* pl = reinterpret_cast<const float4*>(sStat + st * 512) + cw0 / 4;   // lse2 of the step's 64 queries
+        const float4* pd = pl + 16;                                                        // delta
+        if (DKDV) mbar_wait_many(&y_full[st], (g / NST) & 1u, 26);   // the step's lse / delta have landed
+        // causal keep: query >= key.  DKDV: query = c0 + col, key = x0 + r.  DQ: query = x0 + r, key = c0 + col.
+        // Only the two diagonal steps need the mask; `rel` is the diagonal's column inside this thread's slice.
+        const bool diag = DKDV ? (c0 < x0 + 128) : (c0 + 63 > x0);
+        const int rel = x0 + r - c0 - cw0;
+        uint32_t wp[CW / 2], wd[CW / 2];
+        auto body = [&](auto masked) {
+#pragma unroll
+          for (int k4 = 0; k4 < CW / 4; ++k4) {
+            float l2[4] = {my_lse2, my_lse2, my_lse2, my_lse2}, dl[4] = {my_delta, my_delta, my_delta, my_delta};
+            if (DKDV) {
+              const float4 a4 = pl[k4], d4 = pd[k4];
+              l2[0] = a4.x; l2[1] = a4.y; l2[2] = a4.z; l2[3] = a4.w;
+              dl[0] = d4.x; dl[1] = d4.y; dl[2] = d4.z; dl[3] = d4.w;
+            }
+            float pv[4], dv[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int i = 4 * k4 + e;
+              float pr = ex2(fmaf(__uint_as_float(s[i]), c, -l2[e]));
+              if (decltype(masked)::value) {
+                const bool keep = DKDV ? (i >= rel) : (i <= rel);
+                pr = keep ? pr : 0.f;
+              }
+              pv[e] = pr;
+              dv[e] = pr * (__uint_as_float(dp[i]) - dl[e]);
+            }
+            wp[2 * k4] = pack_bf16x2(pv[0], pv[1]); wp[2 * k4 + 1] = pack_bf16x2(pv[2], pv[3]);
+            wd[2 * k4] = pack_bf16x2(dv[0], dv[1]); wd[2 * k4 + 1] = pack_bf16x2(dv[2], dv[3]);
+          }
+        };
+        if (diag) body(std::true_type{}); else body(std::false_type{});
+        if (g > 0) mbar_wait_many(e_empty, (g - 1) & 1u, 27);                  // the previous accumulate MMAs have read E
+        // P^T / dS^T go to TENSOR MEMORY (the thread's lane, CW/2 packed columns each) and are the A operands of the
+        // accumulate MMAs straight from there: no shared-memory round trip, no proxy fence.  dK/dV: they overwrite
+        // this thread's own 32 columns of T1 (already in its registers); dQ: dS has columns of its own.
+        static_assert(CW == 32, "tcgen05.st x16 per thread");
+        if (DKDV) {
+          tmem_st16(tT1 + lane_off + cw0, wp);
+          tmem_st16(tT1 + lane_off + cw0 + 16, wd);
+        } else {
+          tmem_st16(tE + lane_off + cw0 / 2, wd);
+        }
+        tmem_st_wait();
+        tc_fence_before();
+        mbar_arrive(e_full);
+      }
+      // epilogue: accumulators -> bf16 rows of dqkv, 32-column chunks dealt round-robin to the warpgroups
+      mbar_wait_many(acc_full, k & 1u, 28);
+      tc_fence_after();
+      bf16* orow = dqkv + ((size_t)it.row0 + x0 + r) * 3 * D + it.h * DH;
+      constexpr int N_CHUNKS = DKDV ? 4 : 2;              // DKDV: dV lo, dV hi, dK lo, dK hi.  DQ: dQ lo, dQ hi
+      for (int q = wg; q < N_CHUNKS; q += EW) {           // warp-uniform
+        if (DKDV) {
+          const int col = (q < 2 ? 2 * D : D) + (q & 1) * 32;
+          store_chunk((q < 2 ? tA0 : tA1) + (q & 1) * 32, orow + col, q < 2 ? 1.f : inv_sqrt,
+                      Gbias != nullptr ? Gbias + it.h * DH + col : nullptr);
+        } else {
+          store_chunk(tA1 + q * 32, orow + q * 32, inv_sqrt, Gbias != nullptr ? Gbias + it.h * DH + q * 32 : nullptr);
+        }
+      }
+      tc_fence_before();
+      mbar_arrive(acc_empty);                             // the next item's first accumulate MMA may overwrite them
     }
   }
   tc_fence_before();
@@ -592,8 +635,10 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
 // delta[b,h,t] = sum_d dO[b,t,h,d] * O[b,t,h,d]: 8 threads per (b,t,h), one 16-byte vector each
 __global__ void __launch_bounds__(256) attn_delta_tc_kernel(size_t n_vec, int T, int H, const bf16* __restrict__ dout,
                                                             const bf16* __restrict__ o, const float* __restrict__ lse,
-                                                            float* __restrict__ delta, float* __restrict__ lse2) {
+                                                            float* __restrict__ delta, float* __restrict__ lse2,
+                                                            int* __restrict__ work_counters) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < 2) work_counters[i] = 0;                        // item counters of the two persistent backward kernels
   float acc = 0.f;
   if (i < n_vec) {
     float a[8], c[8];
@@ -615,7 +660,8 @@ __global__ void __launch_bounds__(256) attn_delta_tc_kernel(size_t n_vec, int T,
 
 }  // namespace
 
-size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H) { return 2 * (size_t)mu * H * T * sizeof(float); }
+// delta, lse2 (fp32 [mu, H, T] each) and the two work counters of the persistent kernels
+size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H) { return 2 * (size_t)mu * H * T * sizeof(float) + 64; }
 
 int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
                      void* dqkv, float* scratch, float* Gbias, cudaStream_t s) {
@@ -635,16 +681,25 @@ int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, co
   }
   float* delta = scratch;
   float* lse2 = scratch + (size_t)mu * H * T;
+  int* counters = reinterpret_cast<int*>(scratch + 2 * (size_t)mu * H * T);
   const size_t n_vec = (size_t)mu * T * D / 8;
   PACI_LAUNCH(attn_delta_tc_kernel, ceil_div((long long)n_vec, 256), 256, 0, s, n_vec, T, H, (const bf16*)dout,
-              (const bf16*)o, lse, delta, lse2);
-  const int grid = (T / 128) * H * mu;
+              (const bf16*)o, lse, delta, lse2, counters);
+  static int n_sm = 0;
+  if (n_sm == 0) {
+    int dev = 0;
+    PACI_CUDA_OK(cudaGetDevice(&dev));
+    PACI_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+  }
+  const int items = (T / 128) * H * mu;
+  static const int per_sm = getenv("PACI_ATTN_CTAS") ? atoi(getenv("PACI_ATTN_CTAS")) : 2;
+  const int grid = (per_sm <= 0 || items < per_sm * n_sm) ? items : per_sm * n_sm;   // persistent: two CTAs per SM
   // dK, dV: stationary K_j, V_j (qkv, 128-row boxes); streamed Q_i (qkv), dO_i (dout), 64-row boxes
-  PACI_LAUNCH((attn_bwd_tc_kernel<true, BWD_EW>), grid, BWD_THREADS, bwd_smem(true), s, q128, q128, q64, d64, T, H, lse2, delta,
-              (bf16*)dqkv, Gbias);
+  PACI_LAUNCH((attn_bwd_tc_kernel<true, BWD_EW>), grid, BWD_THREADS, bwd_smem(true), s, q128, q128, q64, d64, T, H, mu, lse2, delta,
+              (bf16*)dqkv, Gbias, counters);
   // dQ: stationary Q_i (qkv), dO_i (dout); streamed K_j, V_j (qkv)
-  PACI_LAUNCH((attn_bwd_tc_kernel<false, BWD_EW>), grid, BWD_THREADS, bwd_smem(false), s, q128, d128, q64, q64, T, H, lse2, delta,
-              (bf16*)dqkv, Gbias);
+  PACI_LAUNCH((attn_bwd_tc_kernel<false, BWD_EW>), grid, BWD_THREADS, bwd_smem(false), s, q128, d128, q64, q64, T, H, mu, lse2, delta,
+              (bf16*)dqkv, Gbias, counters + 1);
   return PACI_OK;
 }
 
