@@ -335,8 +335,9 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   uint64_t* bars = (uint64_t*)(sStat + NST * 512);
   uint64_t *x_full = bars, *y_full = bars + 1, *y_empty = bars + 1 + NST, *t_full = bars + 1 + 2 * NST, *e_full = t_full + 1,
            *e_empty = t_full + 2, *acc_full = t_full + 3, *t_free = t_full + 4, *x_empty = t_full + 5, *acc_empty = t_full + 6,
-           *item_full = t_full + 7;                      // [2]
-  uint32_t* tmem_slot = (uint32_t*)(t_full + 9);
+           *item_full = t_full + 7 /* [2] */, *t1_full = t_full + 9, *t1_free = t_full + 10;
+  // t_full / t_free: T0 (the score tile S) landed / is in registers; t1_full / t1_free: the same for T1 (dP)
+  uint32_t* tmem_slot = (uint32_t*)(t_full + 11);
   volatile int* item_slot = (volatile int*)(tmem_slot + 1);   // [2]
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -365,6 +366,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
     mbar_init(x_full, 1);
     for (int i = 0; i < NST; ++i) { mbar_init(&y_full[i], 1); mbar_init(&y_empty[i], 1); }
     mbar_init(t_full, 1); mbar_init(e_full, 128 * EW); mbar_init(e_empty, 1); mbar_init(acc_full, 1); mbar_init(t_free, 128 * EW);
+    mbar_init(t1_full, 1); mbar_init(t1_free, 128 * EW);
     mbar_init(x_empty, 1); mbar_init(acc_empty, 128 * EW); mbar_init(&item_full[0], 1); mbar_init(&item_full[1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -427,13 +429,14 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)
           umma_bf16(tT0, smem_desc(aX0 + kk * 32, 16, 1024), smem_desc(aY0 + kk * 32, 16, 1024), ID_T, kk > 0 ? 1u : 0u);
+        umma_commit(t_full);
       };
       auto issue_t1 = [&](uint32_t gs) {                  // after issue_t0(gs): the stage is known to have landed
         const uint32_t aY1 = smem_u32(sY + (gs % NST) * YST) + HALF_BYTES;
 #pragma unroll
         for (int kk = 0; kk < 4; ++kk)
           umma_bf16(tT1, smem_desc(aX1 + kk * 32, 16, 1024), smem_desc(aY1 + kk * 32, 16, 1024), ID_T, kk > 0 ? 1u : 0u);
-        umma_commit(t_full);
+        umma_commit(t1_full);
       };
       uint32_t g = 0;
       for (uint32_t k = 0;; ++k) {
@@ -444,6 +447,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
         mbar_wait(x_full, k & 1u, 23);
         if (g > 0) {                                      // the previous item's last T0 / T1 are in registers
           mbar_wait(t_free, (g - 1) & 1u, 29);
+          if (!DKDV) mbar_wait(t1_free, (g - 1) & 1u, 30);   // (dK/dV: implied by e_full, T1 goes behind the accumulates)
           tc_fence_after();
         }
         issue_t0(g);
@@ -459,6 +463,8 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
             tc_fence_after();
             issue_t0(g + 1);
             if (!DKDV) {
+              mbar_wait(t1_free, g & 1u, 30);
+              tc_fence_after();
               issue_t1(g + 1);
               if (t + 2 == n_steps) umma_commit(x_empty); // X is not read again: the next item's may load
             }
@@ -535,8 +541,15 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       }
     };
     uint32_t g = 0;
+#ifdef PACI_ATTN_TIMING
+    long long tk[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tprev = clock64(), tnow;
+#define TICK(i) do { tnow = clock64(); tk[i] += tnow - tprev; tprev = tnow; } while (0)
+#else
+#define TICK(i) do {} while (0)
+#endif
     for (uint32_t k = 0;; ++k) {
       mbar_wait_many(&item_full[k & 1], (k >> 1) & 1u, 17);
+      TICK(5);
       const int item = item_slot[k & 1];
       if (item >= n_items) break;
       const Item it = decode(item);
@@ -548,14 +561,17 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       }
       for (int t = 0; t < it.n_steps; ++t, ++g) {
         const int st = g % NST, c0 = it.c_begin + t * 64;
+        // phase 1 needs only the scores: P = exp2(S c - lse2), masked on the diagonal steps.  It runs while the tensor
+        // pipe is still busy with the previous step's accumulate MMAs and this step's T1 (which, for dK/dV, can only
+        // be issued behind them).
         mbar_wait_many(t_full, g & 1u, 25);
         tc_fence_after();
-        uint32_t s[CW], dp[CW];
+        TICK(0);
+        uint32_t s[CW];                                   // S, then P (fp32 bits)
         tmem_ld_cols_nowait<CW>(tT0 + lane_off + cw0, s);
-        tmem_ld_cols_nowait<CW>(tT1 + lane_off + cw0, dp);
         tmem_ld_wait();
         tc_fence_before();
-        mbar_arrive(t_free);                              // T0 / T1 may be overwritten by the next step's MMAs
+        mbar_arrive(t_free);                              // T0 may be overwritten by the next step's score MMA
         const float4* pl = reinterpret_cast<const float4*>(sStat + st * 512) + cw0 / 4;   // lse2 of the step's 64 queries
         const float4* pd = pl + 16;                                                        // delta
         if (DKDV) mbar_wait_many(&y_full[st], (g / NST) & 1u, 26);   // the step's lse / delta have landed
@@ -564,16 +580,14 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
         const bool diag = DKDV ? (c0 < x0 + 128) : (c0 + 63 > x0);
         const int rel = x0 + r - c0 - cw0;
         uint32_t wp[CW / 2], wd[CW / 2];
-        auto body = [&](auto masked) {
+        auto phase1 = [&](auto masked) {
 #pragma unroll
           for (int k4 = 0; k4 < CW / 4; ++k4) {
-            float l2[4] = {my_lse2, my_lse2, my_lse2, my_lse2}, dl[4] = {my_delta, my_delta, my_delta, my_delta};
+            float l2[4] = {my_lse2, my_lse2, my_lse2, my_lse2};
             if (DKDV) {
-              const float4 a4 = pl[k4], d4 = pd[k4];
+              const float4 a4 = pl[k4];
               l2[0] = a4.x; l2[1] = a4.y; l2[2] = a4.z; l2[3] = a4.w;
-              dl[0] = d4.x; dl[1] = d4.y; dl[2] = d4.z; dl[3] = d4.w;
             }
-            float pv[4], dv[4];
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
               const int i = 4 * k4 + e;
@@ -582,15 +596,48 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
                 const bool keep = DKDV ? (i >= rel) : (i <= rel);
                 pr = keep ? pr : 0.f;
               }
-              pv[e] = pr;
-              dv[e] = pr * (__uint_as_float(dp[i]) - dl[e]);
+              s[i] = __float_as_uint(pr);
             }
-            wp[2 * k4] = pack_bf16x2(pv[0], pv[1]); wp[2 * k4 + 1] = pack_bf16x2(pv[2], pv[3]);
-            wd[2 * k4] = pack_bf16x2(dv[0], dv[1]); wd[2 * k4 + 1] = pack_bf16x2(dv[2], dv[3]);
+            if (DKDV) {
+              wp[2 * k4] = pack_bf16x2(__uint_as_float(s[4 * k4]), __uint_as_float(s[4 * k4 + 1]));
+              wp[2 * k4 + 1] = pack_bf16x2(__uint_as_float(s[4 * k4 + 2]), __uint_as_float(s[4 * k4 + 3]));
+            }
           }
         };
-        if (diag) body(std::true_type{}); else body(std::false_type{});
+        if (diag) phase1(std::true_type{}); else phase1(std::false_type{});
+        TICK(1);
+        // phase 2: dS = P o (dP - delta), in two halves to keep the register footprint down
+        mbar_wait_many(t1_full, g & 1u, 31);
+        tc_fence_after();
+        TICK(2);
+#pragma unroll
+        for (int hf = 0; hf < 2; ++hf) {
+          uint32_t dp[CW / 2];
+          tmem_ld_cols_nowait<CW / 2>(tT1 + lane_off + cw0 + hf * (CW / 2), dp);
+          tmem_ld_wait();
+#pragma unroll
+          for (int k4 = 0; k4 < CW / 8; ++k4) {
+            float dl[4] = {my_delta, my_delta, my_delta, my_delta};
+            if (DKDV) {
+              const float4 d4 = pd[hf * (CW / 8) + k4];
+              dl[0] = d4.x; dl[1] = d4.y; dl[2] = d4.z; dl[3] = d4.w;
+            }
+            float dv[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int i = 4 * k4 + e;
+              dv[e] = __uint_as_float(s[hf * (CW / 2) + i]) * (__uint_as_float(dp[i]) - dl[e]);
+            }
+            wd[hf * (CW / 4) + 2 * k4] = pack_bf16x2(dv[0], dv[1]);
+            wd[hf * (CW / 4) + 2 * k4 + 1] = pack_bf16x2(dv[2], dv[3]);
+          }
+        }
+        if (!DKDV) {                                      // (dK/dV: e_full says as much)
+          tc_fence_before();
+          mbar_arrive(t1_free);                           // T1 may be overwritten by the next step's dP MMA
+        }
         if (g > 0) mbar_wait_many(e_empty, (g - 1) & 1u, 27);                  // the previous accumulate MMAs have read E
+        TICK(3);
         // P^T / dS^T go to TENSOR MEMORY (the thread's lane, CW/2 packed columns each) and are the A operands of the
         // accumulate MMAs straight from there: no shared-memory round trip, no proxy fence.  dK/dV: they overwrite
         // this thread's own 32 columns of T1 (already in its registers); dQ: dS has columns of its own.
@@ -604,10 +651,12 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
         tmem_st_wait();
         tc_fence_before();
         mbar_arrive(e_full);
+        TICK(4);
       }
       // epilogue: accumulators -> bf16 rows of dqkv, 32-column chunks dealt round-robin to the warpgroups
       mbar_wait_many(acc_full, k & 1u, 28);
       tc_fence_after();
+      TICK(6);
       bf16* orow = dqkv + ((size_t)it.row0 + x0 + r) * 3 * D + it.h * DH;
       constexpr int N_CHUNKS = DKDV ? 4 : 2;              // DKDV: dV lo, dV hi, dK lo, dK hi.  DQ: dQ lo, dQ hi
       for (int q = wg; q < N_CHUNKS; q += EW) {           // warp-uniform
@@ -621,7 +670,13 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
       }
       tc_fence_before();
       mbar_arrive(acc_empty);                             // the next item's first accumulate MMA may overwrite them
+      TICK(7);
     }
+#ifdef PACI_ATTN_TIMING
+    if (threadIdx.x == 64 && (blockIdx.x == 0 || blockIdx.x == 150 || blockIdx.x == 295))
+      printf("bwd dkdv=%d blk %d steps %u items: per step: wait_t0 %lld phase1 %lld wait_t1 %lld phase2+wait_e %lld st+arrive %lld | total: item_wait %lld acc_wait %lld epilogue %lld\n",
+             (int)DKDV, (int)blockIdx.x, g, tk[0] / g, tk[1] / g, tk[2] / g, tk[3] / g, tk[4] / g, tk[5], tk[6], tk[7]);
+#endif
   }
   tc_fence_before();
   __syncthreads();
