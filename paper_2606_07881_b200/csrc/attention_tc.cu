@@ -542,14 +542,14 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
     };
     uint32_t g = 0;
 #ifdef PACI_ATTN_TIMING
-    long long tk[8] = {0, 0, 0, 0, 0, 0, 0, 0}, tprev = clock64(), tnow;
+    long long tk[10] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tprev = clock64(), tnow;
 #define TICK(i) do { tnow = clock64(); tk[i] += tnow - tprev; tprev = tnow; } while (0)
 #else
 #define TICK(i) do {} while (0)
 #endif
     for (uint32_t k = 0;; ++k) {
       mbar_wait_many(&item_full[k & 1], (k >> 1) & 1u, 17);
-      TICK(5);
+      TICK((k == 0 ? 8 : 5));
       const int item = item_slot[k & 1];
       if (item >= n_items) break;
       const Item it = decode(item);
@@ -566,7 +566,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
         // be issued behind them).
         mbar_wait_many(t_full, g & 1u, 25);
         tc_fence_after();
-        TICK(0);
+        TICK((t == 0 ? (k == 0 ? 8 : 9) : 0));
         uint32_t s[CW];                                   // S, then P (fp32 bits)
         tmem_ld_cols_nowait<CW>(tT0 + lane_off + cw0, s);
         tmem_ld_wait();
@@ -674,8 +674,8 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
     }
 #ifdef PACI_ATTN_TIMING
     if (threadIdx.x == 64 && (blockIdx.x == 0 || blockIdx.x == 150 || blockIdx.x == 295))
-      printf("bwd dkdv=%d blk %d steps %u items: per step: wait_t0 %lld phase1 %lld wait_t1 %lld phase2+wait_e %lld st+arrive %lld | total: item_wait %lld acc_wait %lld epilogue %lld\n",
-             (int)DKDV, (int)blockIdx.x, g, tk[0] / g, tk[1] / g, tk[2] / g, tk[3] / g, tk[4] / g, tk[5], tk[6], tk[7]);
+      printf("bwd dkdv=%d blk %d steps %u items: per step: wait_t0 %lld phase1 %lld wait_t1 %lld phase2+wait_e %lld st+arrive %lld | total: prologue %lld item_wait %lld first_t0 %lld acc_wait %lld epilogue %lld\n",
+             (int)DKDV, (int)blockIdx.x, g, tk[0] / g, tk[1] / g, tk[2] / g, tk[3] / g, tk[4] / g, tk[8], tk[5], tk[9], tk[6], tk[7]);
 #endif
   }
   tc_fence_before();
