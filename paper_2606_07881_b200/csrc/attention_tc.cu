@@ -518,6 +518,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
     auto store_chunk = [&](uint32_t taddr, bf16* dst, float scale, float* gcol) {   // 32 fp32 columns -> 32 bf16
       uint32_t ov[32];
       tmem_ld32(taddr + lane_off, ov);
+      float cs[32];                                       // the rounded values, for the column sums
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
         uint4 w;
@@ -526,18 +527,28 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
         w.z = pack_bf16x2(__uint_as_float(ov[8 * i + 4]) * scale, __uint_as_float(ov[8 * i + 5]) * scale);
         w.w = pack_bf16x2(__uint_as_float(ov[8 * i + 6]) * scale, __uint_as_float(ov[8 * i + 7]) * scale);
         *reinterpret_cast<uint4*>(dst + i * 8) = w;
-        if (gcol != nullptr) {
-          const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
+        const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
 #pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            const float lo = warp_sum(__uint_as_float(ww[u] << 16));
-            const float hi = warp_sum(__uint_as_float(ww[u] & 0xffff0000u));
-            if (lane == 0) {
-              atomicAdd(gcol + 8 * i + 2 * u, lo);
-              atomicAdd(gcol + 8 * i + 2 * u + 1, hi);
-            }
+        for (int u = 0; u < 4; ++u) {
+          cs[8 * i + 2 * u] = __uint_as_float(ww[u] << 16);
+          cs[8 * i + 2 * u + 1] = __uint_as_float(ww[u] & 0xffff0000u);
+        }
+      }
+      if (gcol != nullptr) {
+        // transposing butterfly: after the step with offset `off` a lane keeps the half of its columns selected by
+        // that bit of its lane id, summed with its partner's; 16 + 8 + 4 + 2 + 1 shuffles leave lane l with the sum
+        // of column l over the warp's 32 rows -> one coalesced atomic per warp
+#pragma unroll
+        for (int off = 16; off >= 1; off >>= 1) {
+          const bool up = (lane & off) != 0;
+#pragma unroll
+          for (int i = 0; i < off; ++i) {
+            const float keep = up ? cs[i + off] : cs[i];
+            const float send = up ? cs[i] : cs[i + off];
+            cs[i] = keep + __shfl_xor_sync(0xffffffffu, send, off);
           }
         }
+        atomicAdd(gcol + lane, cs[0]);
       }
     };
     uint32_t g = 0;
