@@ -3,6 +3,8 @@
 // reductions; grids are sized from the SM count.
 #include <cmath>
 #include <cstdarg>
+#include <cstdlib>
+#include <string>
 
 #include "common.cuh"
 
@@ -391,6 +393,176 @@ __global__ void __launch_bounds__(NW * 32) ln_bwd_fused_kernel(int rows, int D, 
   }
 }
 
+// Pipelined variant of the single-pass kernel: one producer thread per block streams LNP_R-row groups of dy, x
+// (and dres) plus their mean / rstd into an S-stage shared-memory ring with bulk async copies (one copy per tensor
+// per group: the rows of a group are contiguous), so the NW compute warps never wait on a global load -- the
+// register-resident version above keeps the loads and the arithmetic of one group in series (26 us, 24% of DRAM
+// peak at 20% occupancy).  The compute warps pull a group into registers, hand the stage back at once, and carry
+// on exactly as above.  Requires rows % LNP_R == 0 and 16-byte aligned mean / rstd.
+constexpr int LNP_R = 4;
+__device__ __forceinline__ uint32_t lnp_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void lnp_bulk_load(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(lnp_smem_u32(dst)), "l"(src), "r"(bytes), "r"(lnp_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void lnp_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n.reg .pred p;\nLNP_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 1000;\n"
+      "@p bra LNP_DONE;\nbra LNP_WAIT;\nLNP_DONE:\n}" ::"r"(lnp_smem_u32(bar)), "r"(parity) : "memory");
+}
+
+template <typename T, int NW, int S, int SETS, int RS>
+__global__ void __launch_bounds__((SETS * NW + 1) * 32, SETS > 1 ? 1 : 2) ln_bwd_pipe_kernel(int rows, int D, const T* __restrict__ dy,
+                                                                   const T* __restrict__ x, const float* __restrict__ mean,
+                                                                   const float* __restrict__ rstd,
+                                                                   const float* __restrict__ g, const T* __restrict__ dres,
+                                                                   T* __restrict__ dx, float* __restrict__ Gg,
+                                                                   float* __restrict__ Gb, float* __restrict__ Gcol) {
+  constexpr int V = Vec<T>::N;
+  constexpr uint32_t RB = NW * 32 * V * sizeof(T);        // bytes of one row
+  constexpr uint32_t TB = LNP_R * RB;                     // one tensor's share of a stage
+  constexpr uint32_t STAGE = 3 * TB + 32;                 // dy, x, dres, mean[R], rstd[R]
+  extern __shared__ __align__(128) uint8_t lnp_smem[];
+  uint64_t* full = reinterpret_cast<uint64_t*>(lnp_smem + S * STAGE);
+  uint64_t* empty = full + S;
+  float (*part)[LNP_R][2][NW] = reinterpret_cast<float (*)[LNP_R][2][NW]>(empty + S);   // [2 * SETS]
+  const int lane = threadIdx.x & 31, w = (threadIdx.x >> 5) % NW, set = (threadIdx.x >> 5) / NW;   // set == SETS: producer
+  const int groups = rows / LNP_R;
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < S; ++i) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(lnp_smem_u32(&full[i])), "r"(1));
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(lnp_smem_u32(&empty[i])), "r"(NW));
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (set == SETS) {                                      // producer
+    if (lane == 0) {
+      uint32_t it = 0;
+      for (int gi = blockIdx.x; gi < groups; gi += gridDim.x, ++it) {
+        const uint32_t st = it % S;
+        lnp_wait(&empty[st], ((it / S) & 1u) ^ 1u);
+        uint8_t* base = lnp_smem + st * STAGE;
+        const size_t off = (size_t)gi * LNP_R * (NW * 32 * V);
+        const uint32_t bytes = (dres != nullptr ? 3u : 2u) * TB + 32u;
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(lnp_smem_u32(&full[st])), "r"(bytes) : "memory");
+        lnp_bulk_load(base, dy + off, TB, &full[st]);
+        lnp_bulk_load(base + TB, x + off, TB, &full[st]);
+        if (dres != nullptr) lnp_bulk_load(base + 2 * TB, dres + off, TB, &full[st]);
+        lnp_bulk_load(base + 3 * TB, mean + (size_t)gi * LNP_R, 16, &full[st]);
+        lnp_bulk_load(base + 3 * TB + 16, rstd + (size_t)gi * LNP_R, 16, &full[st]);
+      }
+    }
+    return;
+  }
+  const int c = (w * 32 + lane) * V;                      // this lane's columns
+  float gg[V], ag[V], ab[V], ac[V];
+  load_f32<V>(g + c, gg);
+#pragma unroll
+  for (int j = 0; j < V; ++j) ag[j] = ab[j] = ac[j] = 0.f;
+  const float invD = 1.f / (float)D;
+  // SETS groups of NW compute warps take alternate row groups off the ring (so the shuffle / barrier latency of one
+  // group hides behind the others') and walk a group RS rows at a time (registers)
+  uint32_t it = set, hb = 0;
+  for (int gi = blockIdx.x + set * gridDim.x; gi < groups; gi += SETS * gridDim.x, it += SETS) {
+    const uint32_t st = it % S;
+    lnp_wait(&full[st], (it / S) & 1u);
+    const uint8_t* base = lnp_smem + st * STAGE;
+#pragma unroll 1
+    for (int h0 = 0; h0 < LNP_R; h0 += RS, hb ^= 1u) {
+    const uint32_t buf = set * 2 + hb;
+    const int r0 = gi * LNP_R + h0;
+    uint4 rdy[RS], rx[RS], rr[RS];
+    float mu[RS], rs[RS];
+#pragma unroll
+    for (int u = 0; u < RS; ++u) {
+      const uint32_t o = (h0 + u) * RB + (uint32_t)c * sizeof(T);
+      rdy[u] = *reinterpret_cast<const uint4*>(base + o);
+      rx[u] = *reinterpret_cast<const uint4*>(base + TB + o);
+      if (dres != nullptr) rr[u] = *reinterpret_cast<const uint4*>(base + 2 * TB + o);
+      mu[u] = *reinterpret_cast<const float*>(base + 3 * TB + 4 * (h0 + u));
+      rs[u] = *reinterpret_cast<const float*>(base + 3 * TB + 16 + 4 * (h0 + u));
+    }
+    if (h0 + RS == LNP_R) {                               // the group is in registers: hand the stage back
+      __syncwarp();
+      if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(lnp_smem_u32(&empty[st])) : "memory");
+    }
+#pragma unroll
+    for (int u = 0; u < RS; ++u) {
+      float dyv[V], xv[V];
+      unpack_raw<T>(rdy[u], dyv);
+      unpack_raw<T>(rx[u], xv);
+      float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+      for (int j = 0; j < V; ++j) {
+        const float gd = dyv[j] * gg[j];
+        s1 += gd;
+        s2 += gd * ((xv[j] - mu[u]) * rs[u]);
+      }
+      s1 = warp_sum(s1);
+      s2 = warp_sum(s2);
+      if (lane == 0) { part[buf][u][0][w] = s1; part[buf][u][1][w] = s2; }
+    }
+    asm volatile("bar.sync %0, %1;" ::"r"(1 + set), "n"(NW * 32) : "memory");   // this set's compute warps only
+#pragma unroll
+    for (int u = 0; u < RS; ++u) {
+      float s1 = 0.f, s2 = 0.f;
+#pragma unroll
+      for (int k = 0; k < NW; ++k) { s1 += part[buf][u][0][k]; s2 += part[buf][u][1][k]; }
+      s1 *= invD;
+      s2 *= invD;
+      float dyv[V], xv[V], o[V];
+      unpack_raw<T>(rdy[u], dyv);
+      unpack_raw<T>(rx[u], xv);
+#pragma unroll
+      for (int j = 0; j < V; ++j) {
+        const float xh = (xv[j] - mu[u]) * rs[u];
+        o[j] = rs[u] * (dyv[j] * gg[j] - s1 - xh * s2);
+        ag[j] += dyv[j] * xh;
+        ab[j] += dyv[j];
+      }
+      if (dres != nullptr) {
+        float rv[V];
+        unpack_raw<T>(rr[u], rv);
+#pragma unroll
+        for (int j = 0; j < V; ++j) o[j] += rv[j];
+      }
+      store_vec<T>(dx + (size_t)(r0 + u) * D + c, o);
+      if (Gcol != nullptr) {
+#pragma unroll
+        for (int j = 0; j < V; ++j) ac[j] += to_f(from_f<T>(o[j]));   // sum of what was stored
+      }
+    }
+    }
+  }
+  // same-address atomics serialise in L2 (~27 cycles each), so the sets first add their partials in shared memory
+  // (the ring is drained) and each block issues ONE vector atomic per 4 columns
+  if (SETS > 1) {
+    float* red = reinterpret_cast<float*>(lnp_smem);      // [SETS - 1][3][D]
+    asm volatile("bar.sync 15, %0;" ::"n"(SETS * NW * 32) : "memory");   // every set is done with the ring
+    if (set > 0) {
+      float* dst = red + (size_t)(set - 1) * 3 * D + c;
+#pragma unroll
+      for (int j = 0; j < V; ++j) { dst[j] = ag[j]; dst[D + j] = ab[j]; dst[2 * D + j] = ac[j]; }
+    }
+    asm volatile("bar.sync 15, %0;" ::"n"(SETS * NW * 32) : "memory");
+    if (set > 0) return;
+#pragma unroll
+    for (int q = 0; q < SETS - 1; ++q) {
+      const float* src = red + (size_t)q * 3 * D + c;
+#pragma unroll
+      for (int j = 0; j < V; ++j) { ag[j] += src[j]; ab[j] += src[D + j]; ac[j] += src[2 * D + j]; }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < V; j += 4) {
+    red_add_v4(Gg + c + j, ag[j], ag[j + 1], ag[j + 2], ag[j + 3]);
+    red_add_v4(Gb + c + j, ab[j], ab[j + 1], ab[j + 2], ab[j + 3]);
+    if (Gcol != nullptr) red_add_v4(Gcol + c + j, ac[j], ac[j + 1], ac[j + 2], ac[j + 3]);
+  }
+}
+
 template <typename T>
 static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float* mean, const float* rstd,
                     const float* g, const void* dres, void* dx, float* Gg, float* Gb, float* Gcol,
@@ -400,6 +572,27 @@ static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float*
   if (D % (32 * V) == 0 && D / (32 * V) <= 8 && (uintptr_t)Gg % 16 == 0 && (uintptr_t)Gb % 16 == 0 &&
       (Gcol == nullptr || (uintptr_t)Gcol % 16 == 0)) {
     const int nw = D / (32 * V);
+    // the shape the stage runs at (bf16, D = 1024): the bulk-copy pipelined kernel, one block per SM (8-stage ring of
+    // 4-row groups = 197 KB, 3 sets of 4 compute warps, 2 rows at a time); PACI_LN_BWD=regs keeps the kernel below
+    if constexpr (sizeof(T) == 2) {
+      static const bool use_pipe = !(getenv("PACI_LN_BWD") && std::string(getenv("PACI_LN_BWD")) == "regs");
+      if (use_pipe && nw == 4 && rows % LNP_R == 0 && (uintptr_t)mean % 16 == 0 && (uintptr_t)rstd % 16 == 0 &&
+          (uintptr_t)dy % 16 == 0 && (uintptr_t)x % 16 == 0 && (uintptr_t)dres % 16 == 0) {
+        constexpr int S = 8, SETS = 3;
+        auto kern = ln_bwd_pipe_kernel<T, 4, S, SETS, 2>;
+        const uint32_t stage = 3 * LNP_R * (uint32_t)D * sizeof(T) + 32;
+        const uint32_t smem = S * stage + 2 * S * 8 + 2 * SETS * LNP_R * 2 * 4 * 4 + 64;
+        static bool attr_set = false;
+        if (!attr_set) {
+          PACI_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+          attr_set = true;
+        }
+        const int blocks = std::min(rows / LNP_R, num_sms());
+        PACI_LAUNCH(kern, blocks, (4 * SETS + 1) * 32, smem, s, rows, D, (const T*)dy, (const T*)x, mean, rstd, g,
+                    (const T*)dres, (T*)dx, Gg, Gb, Gcol);
+        return PACI_OK;
+      }
+    }
     const int blocks = std::min(ceil_div(rows, LNF_R), num_sms() * std::max(1, 16 / nw));
 #define LNF_CASE(N)                                                                                      \
   case N:                                                                                                \
