@@ -112,11 +112,146 @@ __global__ void __launch_bounds__(256) ln_fwd_kernel(int rows, int D, const T* _
   }
 }
 
+// Pipelined forward for the stage's shape (bf16, D = 1024): one block per SM; a producer thread streams 4-row groups
+// of x (and the residual) into a 12-stage shared-memory ring with bulk async copies, 3 sets of 4 compute warps take
+// alternate groups, one warp per row as above; gamma / beta stay in registers.  The one-wave kernel above issues
+// every load, then every store (15.5 us under ncu); here loads, arithmetic and stores of different groups overlap.
+constexpr int LNQ_R = 4;
+template <typename T, int S, int SETS>
+__global__ void __launch_bounds__((SETS * LNQ_R + 1) * 32, 1) ln_fwd_pipe_kernel(int rows, const T* __restrict__ x,
+                                                                                const T* __restrict__ res,
+                                                                                const float* __restrict__ g,
+                                                                                const float* __restrict__ b,
+                                                                                T* __restrict__ xsum, T* __restrict__ y,
+                                                                                float* __restrict__ mean_out,
+                                                                                float* __restrict__ rstd_out) {
+  constexpr int V = Vec<T>::N, NV = 4, D = NV * 32 * V;
+  constexpr uint32_t RB = D * sizeof(T), TB = LNQ_R * RB, STAGE = 2 * TB;
+  extern __shared__ __align__(128) uint8_t lnq_smem[];
+  uint64_t* full = reinterpret_cast<uint64_t*>(lnq_smem + S * STAGE);
+  uint64_t* empty = full + S;
+  const int lane = threadIdx.x & 31, w = (threadIdx.x >> 5) % LNQ_R, set = (threadIdx.x >> 5) / LNQ_R;
+  const int groups = rows / LNQ_R;
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < S; ++i) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&full[i])), "r"(1));
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(&empty[i])), "r"(LNQ_R));
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  auto wait = [](uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n.reg .pred p;\nLNQ_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 1000;\n"
+        "@p bra LNQ_DONE;\nbra LNQ_WAIT;\nLNQ_DONE:\n}" ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
+  };
+  if (set == SETS) {                                      // producer
+    if (lane == 0) {
+      uint32_t it = 0;
+      for (int gi = blockIdx.x; gi < groups; gi += gridDim.x, ++it) {
+        const uint32_t st = it % S;
+        wait(&empty[st], ((it / S) & 1u) ^ 1u);
+        uint8_t* base = lnq_smem + st * STAGE;
+        const size_t off = (size_t)gi * LNQ_R * D;
+        const uint32_t fb = (uint32_t)__cvta_generic_to_shared(&full[st]);
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(fb), "r"((res != nullptr ? 2u : 1u) * TB) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                     ::"r"((uint32_t)__cvta_generic_to_shared(base)), "l"(x + off), "r"(TB), "r"(fb) : "memory");
+        if (res != nullptr)
+          asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                       ::"r"((uint32_t)__cvta_generic_to_shared(base + TB)), "l"(res + off), "r"(TB), "r"(fb) : "memory");
+      }
+    }
+    return;
+  }
+  float gg[NV][V], bb[NV][V];
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    load_f32<V>(g + (size_t)(lane + 32 * i) * V, gg[i]);
+    load_f32<V>(b + (size_t)(lane + 32 * i) * V, bb[i]);
+  }
+  uint32_t it = set;
+  for (int gi = blockIdx.x + set * gridDim.x; gi < groups; gi += SETS * gridDim.x, it += SETS) {
+    const uint32_t st = it % S;
+    const int row = gi * LNQ_R + w;
+    const size_t base = (size_t)row * D;
+    wait(&full[st], (it / S) & 1u);
+    const uint8_t* sx = lnq_smem + st * STAGE + w * RB;
+    uint4 rx[NV], rr[NV];
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      rx[i] = *reinterpret_cast<const uint4*>(sx + (lane + 32 * i) * 16);
+      if (res != nullptr) rr[i] = *reinterpret_cast<const uint4*>(sx + TB + (lane + 32 * i) * 16);
+    }
+    __syncwarp();
+    if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((uint32_t)__cvta_generic_to_shared(&empty[st])) : "memory");
+    float v[NV][V];
+    float sum = 0.f;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      unpack_raw<T>(rx[i], v[i]);
+      if (res != nullptr) {
+        float r[V];
+        unpack_raw<T>(rr[i], r);
+#pragma unroll
+        for (int j = 0; j < V; ++j) v[i][j] += r[j];
+      }
+      if (xsum != nullptr) {
+        store_vec<T>(xsum + base + (size_t)(lane + 32 * i) * V, v[i]);
+#pragma unroll
+        for (int j = 0; j < V; ++j) v[i][j] = to_f(from_f<T>(v[i][j]));   // statistics see the ROUNDED stream
+      }
+#pragma unroll
+      for (int j = 0; j < V; ++j) sum += v[i][j];
+    }
+    const float mean = warp_sum(sum) / (float)D;
+    float sq = 0.f;
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+#pragma unroll
+      for (int j = 0; j < V; ++j) {
+        const float d = v[i][j] - mean;
+        sq += d * d;
+      }
+    }
+    const float rstd = rsqrtf(warp_sum(sq) / (float)D + LN_EPS);
+    if (lane == 0) {
+      mean_out[row] = mean;
+      rstd_out[row] = rstd;
+    }
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      float o[V];
+#pragma unroll
+      for (int j = 0; j < V; ++j) o[j] = (v[i][j] - mean) * rstd * gg[i][j] + bb[i][j];
+      store_vec<T>(y + base + (size_t)(lane + 32 * i) * V, o);
+    }
+  }
+}
+
 template <typename T>
 static int ln_fwd_t(int rows, int D, const void* x, const void* res, const float* g, const float* b,
                     void* xsum, void* y, float* mean, float* rstd, cudaStream_t s) {
   constexpr int V = Vec<T>::N;
   if (D % V != 0) return fail(PACI_EINVAL, "layernorm: D=%d not a multiple of %d", D, V);
+  if constexpr (sizeof(T) == 2) {
+    static const bool use_pipe = !(getenv("PACI_LN_FWD") && std::string(getenv("PACI_LN_FWD")) == "regs");
+    if (use_pipe && D == 1024 && rows % LNQ_R == 0 && (uintptr_t)x % 16 == 0 && (uintptr_t)res % 16 == 0) {
+      constexpr int S = 12, SETS = 3;
+      auto kern = ln_fwd_pipe_kernel<T, S, SETS>;
+      const uint32_t smem = S * 2 * LNQ_R * (uint32_t)D * sizeof(T) + 2 * S * 8 + 64;
+      static bool attr_set = false;
+      if (!attr_set) {
+        PACI_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set = true;
+      }
+      const int blocks = std::min(rows / LNQ_R, num_sms());
+      PACI_LAUNCH(kern, blocks, (SETS * LNQ_R + 1) * 32, smem, s, rows, (const T*)x, (const T*)res, g, b, (T*)xsum, (T*)y,
+                  mean, rstd);
+      return PACI_OK;
+    }
+  }
   const int nv = ceil_div(D / V, 32);
   const int wpb = 8;
   dim3 grid(ceil_div(rows, wpb)), block(wpb * 32);
