@@ -183,6 +183,34 @@ def oracle_sample(c, steps, warmup):
     return mu * T / t, info
 
 
+def oracle_one_thread(c):
+    """SURVEY.md 8(d) also asks for a 1-thread figure: the same oracle, ONE block of the interior stage at full
+    width (micro-batch 1), F + B only, timed with the BLAS pool limited to one thread and again with all threads."""
+    import synth
+    from oracle import model
+    from threadpoolctl import threadpool_limits
+    S, D, H, T, V = c["S"], c["D"], c["H"], c["T"], c["V"]
+    s = 1 if S >= 3 else 0
+    spec = model.StageSpec(s, max(S, 3) if s == 1 else S, 1, D, H, T, 1, V)
+    if spec.has_embedding or spec.has_head:
+        return None
+    theta = {n: np.asarray(a, np.float64) for n, a in synth.stage_params(SEED, s, spec.n_stages, 1, D, V, T).items()}
+    rng = np.random.default_rng(SEED)
+    inp, dout = rng.standard_normal((1, T, D)), rng.standard_normal((1, T, D)) * 1e-3
+
+    def once():
+        t0 = time.perf_counter()
+        _, stash = model.stage_forward(spec, theta, inp, None)
+        model.stage_backward(spec, theta, stash, dout)
+        return time.perf_counter() - t0
+    once()
+    t_all = once()
+    with threadpool_limits(limits=1):
+        t_one = once()
+    return {"value": T / t_one, "unit": UNIT, "cores": 1, "all_cores_value": T / t_all,
+            "sample": f"one block of the interior stage (D={D}, H={H}, T={T}), micro-batch 1, F + B, fp64 numpy oracle"}
+
+
 def run_reference(args, c, name):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -368,6 +396,12 @@ def run_ours(args, c, name):
         val, info = oracle_sample(c, 1, 0)
         line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
                                 "sample": info["sample"]}
+        try:
+            one = oracle_one_thread(c)
+            if one is not None:
+                line["cpu_baseline"]["one_thread"] = one
+        except Exception as e:                       # the 1-thread figure is an extra, never a reason to lose the line
+            line["cpu_baseline"]["one_thread"] = {"unavailable": repr(e)[:200]}
     print(json.dumps(line))
     return 0
 
