@@ -141,3 +141,47 @@ def test_pipeline_full_width_with_drift():
     _compare(out, ref, stages, pb.BF16, n, 5e-3, lr_bound=2 * lr)
     for st in stages:
         st.close()
+
+
+@pytest.mark.parametrize("rows,with_res", [(M, True), (4100, True), (M, False), (600, False)])
+def test_layernorm_pipelined_kernels_full_size(rows, with_res):
+    """The bulk-copy pipelined LayerNorm kernels (bf16, D = 1024: the shape bench.py runs) over enough rows for every
+    block's shared-memory ring to wrap several times (8192 rows = 2048 groups on 148 blocks x 3 warp sets), with a
+    group count that does not divide evenly, and with / without the fused residual, dres and bias-gradient column."""
+    from gpu_util import f32
+    rng = np.random.default_rng(rows)
+    x, res = rng.standard_normal((rows, D)) * 2 + 0.3, rng.standard_normal((rows, D))
+    g, b = 1 + 0.1 * rng.standard_normal(D), 0.1 * rng.standard_normal(D)
+    dy, dres = rng.standard_normal((rows, D)), rng.standard_normal((rows, D))
+    xs_ref = rounded(rounded(x, pb.BF16) + rounded(res, pb.BF16), pb.BF16) if with_res else rounded(x, pb.BF16)
+    y_ref, (xhat, rstd) = model.layernorm_fwd(xs_ref, g.astype(np.float32).astype(np.float64),
+                                              b.astype(np.float32).astype(np.float64))
+    xd, rd, gd, bd = _bf(x), _bf(res), f32(g), f32(b)
+    xsum, y = torch.empty_like(xd), torch.empty_like(xd)
+    mean, rs = torch.empty(rows, device="cuda"), torch.empty(rows, device="cuda")
+    ck(lib.paci_op_layernorm_fwd(pb.BF16, rows, D, xd.data_ptr(), rd.data_ptr() if with_res else None, gd.data_ptr(),
+                                 bd.data_ptr(), xsum.data_ptr() if with_res else None, y.data_ptr(), mean.data_ptr(),
+                                 rs.data_ptr(), S0()))
+    torch.cuda.synchronize()
+    if with_res:
+        assert rel_l2(host(xsum), xs_ref) < 1e-7
+    assert rel_l2(host(y), y_ref) < TOL[pb.BF16] / 4
+    assert rel_l2(host(rs), rstd[:, 0]) < 1e-5 and rel_l2(host(mean), xs_ref.mean(-1)) < 1e-5
+    g2 = g + 0.05 * rng.standard_normal(D)                   # backward with the CURRENT gain (Eq. 1)
+    dx_ref, dg_ref, db_ref = model.layernorm_bwd(rounded(dy, pb.BF16), (xhat, rstd), g2.astype(np.float32).astype(np.float64))
+    if with_res:
+        dx_ref = dx_ref + rounded(dres, pb.BF16)
+    dx = torch.empty_like(xd)
+    Gg = torch.full((D,), 0.5, device="cuda"); Gb = torch.full((D,), -0.25, device="cuda")
+    Gc = torch.full((D,), 1.0, device="cuda")
+    src = xsum if with_res else xd
+    dyd, dresd, g2d = _bf(dy), _bf(dres), f32(g2)             # named: the buffers must outlive the launch
+    ck(lib.paci_op_layernorm_bwd(pb.BF16, rows, D, dyd.data_ptr(), src.data_ptr(), mean.data_ptr(), rs.data_ptr(),
+                                 g2d.data_ptr(), dresd.data_ptr() if with_res else None, dx.data_ptr(),
+                                 Gg.data_ptr(), Gb.data_ptr(), Gc.data_ptr() if with_res else None, S0()))
+    torch.cuda.synchronize()
+    assert rel_l2(host(dx), dx_ref) < TOL[pb.BF16] / 4
+    assert rel_l2(host(Gg) - 0.5, dg_ref) < TOL[pb.BF16] / 4
+    assert rel_l2(host(Gb) + 0.25, db_ref) < TOL[pb.BF16] / 4
+    if with_res:
+        assert rel_l2(host(Gc) - 1.0, host(dx).astype(np.float64).sum(0)) < 1e-4

@@ -81,8 +81,9 @@ def test_layernorm_fwd_bwd(dtype, rows, D):
     dx = torch.empty_like(xd)
     Gg = torch.full((D,), 0.5, device="cuda"); Gb = torch.full((D,), -0.25, device="cuda")
     Gc = torch.full((D,), 1.0, device="cuda")
-    ck(lib.paci_op_layernorm_bwd(dtype, rows, D, dev(dy, dtype).data_ptr(), xsum.data_ptr(), mean.data_ptr(),
-                                 rs.data_ptr(), f32(g2).data_ptr(), dev(dres, dtype).data_ptr(), dx.data_ptr(),
+    dyd, dresd, g2d = dev(dy, dtype), dev(dres, dtype), f32(g2)      # named: the buffers must outlive the launch
+    ck(lib.paci_op_layernorm_bwd(dtype, rows, D, dyd.data_ptr(), xsum.data_ptr(), mean.data_ptr(),
+                                 rs.data_ptr(), g2d.data_ptr(), dresd.data_ptr(), dx.data_ptr(),
                                  Gg.data_ptr(), Gb.data_ptr(), Gc.data_ptr(), S0))
     assert rel_l2(host(dx), dx_ref) < TOL[dtype] / 4
     assert rel_l2(host(Gg) - 0.5, dg_ref) < TOL[dtype] / 4          # accumulates INTO G (beta = 1)
@@ -100,8 +101,9 @@ def test_gemm_bias_gelu(dtype, M, N, K):
     p_ref, _ = model.linear_fwd(xr, Wr, b.astype(np.float32).astype(np.float64))
     Cd = torch.empty(M, N, device="cuda", dtype=DT[dtype])
     Gd = torch.empty(M, N, device="cuda", dtype=DT[dtype])
-    ck(lib.paci_op_gemm_bias_gelu(dtype, M, N, K, dev(x, dtype).data_ptr(), K, dev(W, dtype).data_ptr(), K,
-                                  f32(b).data_ptr(), Cd.data_ptr(), Gd.data_ptr(), N, S0))
+    xd, Wd, bd = dev(x, dtype), dev(W, dtype), f32(b)
+    ck(lib.paci_op_gemm_bias_gelu(dtype, M, N, K, xd.data_ptr(), K, Wd.data_ptr(), K,
+                                  bd.data_ptr(), Cd.data_ptr(), Gd.data_ptr(), N, S0))
     assert rel_l2(host(Cd), p_ref) < TOL[dtype] / 4
     assert rel_l2(host(Gd), model.gelu_fwd(host(Cd))) < TOL[dtype] / 4      # gelu of what was stored
     assert rel_l2(host(Gd), model.gelu_fwd(p_ref)) < TOL[dtype] / 2
@@ -141,7 +143,8 @@ def test_embedding_fwd_bwd_zipf(dtype):
     wte, wpe = rng.standard_normal((V, D)).astype(np.float32), rng.standard_normal((T, D)).astype(np.float32)
     tokd = torch.from_numpy(tok).cuda()
     x = torch.empty(mu, T, D, device="cuda", dtype=DT[dtype])
-    ck(lib.paci_op_embed_fwd(dtype, mu, T, D, tokd.data_ptr(), f32(wte).data_ptr(), f32(wpe).data_ptr(),
+    wted, wped = f32(wte), f32(wpe)
+    ck(lib.paci_op_embed_fwd(dtype, mu, T, D, tokd.data_ptr(), wted.data_ptr(), wped.data_ptr(),
                              x.data_ptr(), S0))
     assert rel_l2(host(x), model.embed_fwd(tok.astype(np.int64), wte.astype(np.float64), wpe.astype(np.float64))) \
         < TOL[dtype] / 4
