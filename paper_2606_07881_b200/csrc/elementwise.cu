@@ -7,6 +7,7 @@
 #include <string>
 
 #include "common.cuh"
+#include "tc_ptx.cuh"
 
 namespace paci {
 
@@ -140,12 +141,7 @@ __global__ void __launch_bounds__((SETS * LNQ_R + 1) * 32, 1) ln_fwd_pipe_kernel
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  auto wait = [](uint64_t* bar, uint32_t parity) {
-    asm volatile(
-        "{\n.reg .pred p;\nLNQ_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 1000;\n"
-        "@p bra LNQ_DONE;\nbra LNQ_WAIT;\nLNQ_DONE:\n}" ::"r"((uint32_t)__cvta_generic_to_shared(bar)), "r"(parity) : "memory");
-  };
+  auto wait = [](uint64_t* bar, uint32_t parity) { tc::mbar_wait_many(bar, parity, 41); };
   if (set == SETS) {                                      // producer
     if (lane == 0) {
       uint32_t it = 0;
@@ -541,10 +537,7 @@ __device__ __forceinline__ void lnp_bulk_load(void* dst, const void* src, uint32
                ::"r"(lnp_smem_u32(dst)), "l"(src), "r"(bytes), "r"(lnp_smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void lnp_wait(uint64_t* bar, uint32_t parity) {
-  asm volatile(
-      "{\n.reg .pred p;\nLNP_WAIT:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, 1000;\n"
-      "@p bra LNP_DONE;\nbra LNP_WAIT;\nLNP_DONE:\n}" ::"r"(lnp_smem_u32(bar)), "r"(parity) : "memory");
+  tc::mbar_wait_many(bar, parity, 40);                    // parked try_wait; traps after 4 s instead of hanging
 }
 
 template <typename T, int NW, int S, int SETS, int RS>
@@ -713,7 +706,10 @@ static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float*
       static const bool use_pipe = !(getenv("PACI_LN_BWD") && std::string(getenv("PACI_LN_BWD")) == "regs");
       if (use_pipe && nw == 4 && rows % LNP_R == 0 && (uintptr_t)mean % 16 == 0 && (uintptr_t)rstd % 16 == 0 &&
           (uintptr_t)dy % 16 == 0 && (uintptr_t)x % 16 == 0 && (uintptr_t)dres % 16 == 0) {
-        constexpr int S = 8, SETS = 3;
+        // S is a multiple of SETS: every ring stage then belongs to ONE set, so each `full` barrier has a single
+        // consumer sequence and a waiter can never be two phases behind it (parity waits cannot tell those apart)
+        constexpr int S = 9, SETS = 3;
+        static_assert(S % SETS == 0, "one owner set per stage");
         auto kern = ln_bwd_pipe_kernel<T, 4, S, SETS, 2>;
         const uint32_t stage = 3 * LNP_R * (uint32_t)D * sizeof(T) + 32;
         const uint32_t smem = S * stage + 2 * S * 8 + 2 * SETS * LNP_R * 2 * 4 * 4 + 64;
