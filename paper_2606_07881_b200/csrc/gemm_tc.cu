@@ -53,6 +53,7 @@ using namespace tc;
 struct Params {
   int M, N, K, ldc;
   int tiles_m, tiles_n, splits, kb_total;
+  int range_mode;                                   // 1: workers own contiguous ranges of (tile, k-block) units
   const float* bias;
   void* C;
   int gelu;       // !ACCUM only: also store gelu(C) through tmC2 (MLP-up: the pre-activation is stashed, rows a7 + a8)
@@ -124,17 +125,43 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   const int kb_per = (p.kb_total + p.splits - 1) / p.splits;
   const int worker = CG == 2 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
   const int n_workers = CG == 2 ? (int)(gridDim.x >> 1) : (int)gridDim.x;
+  // The work list of this CTA (pair), walked identically by the producer, the MMA issuer and the epilogue warps.
+  // Item mode: items = tile x split, dealt round-robin.  Range mode (fp32 reduce-add output only): the (tile,
+  // k-block) space is cut into n_workers equal contiguous ranges, so every worker does the same number of k-blocks
+  // and flushes its accumulator wherever its range crosses a tile boundary (partials meet in the L2 adders).
+  struct Work {
+    long cur, end;
+    int item, n_items, step, splits, kb_per, kb_total, range;
+    __device__ __forceinline__ bool next(int& tile, int& kb0, int& kb1) {
+      if (range) {
+        if (cur >= end) return false;
+        tile = (int)(cur / kb_total);
+        kb0 = (int)(cur % kb_total);
+        kb1 = (int)min((long)kb_total, kb0 + (end - cur));
+        cur += kb1 - kb0;
+        return true;
+      }
+      if (item >= n_items) return false;
+      tile = item / splits;
+      kb0 = (item % splits) * kb_per;
+      kb1 = min(kb0 + kb_per, kb_total);
+      item += step;
+      return true;
+    }
+  };
+  const long units = (long)p.tiles_m * p.tiles_n * p.kb_total;
+  const Work work0{units * worker / n_workers, units * (worker + 1) / n_workers, worker, n_items, n_workers, p.splits, kb_per,
+                   p.kb_total, p.range_mode};
 
   if (warp == 0) {
     if (lane == 0) {
       asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
       asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
       uint32_t stage = 0, phase = 0;
-      for (int item = worker; item < n_items; item += n_workers) {
-        const int tile = item / p.splits, split = item % p.splits;
+      Work work = work0;
+      for (int tile, kb0, kb1; work.next(tile, kb0, kb1);) {
         const int m0 = (tile % p.tiles_m) * (BLOCK_M * CG) + (int)rank * BLOCK_M;
         const int n0 = (tile / p.tiles_m) * BLOCK_N + (int)rank * BN_CTA;
-        const int kb0 = split * kb_per, kb1 = min(kb0 + kb_per, p.kb_total);
         for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(&empty[stage], phase ^ 1, 1);
           uint8_t* sa = smem + stage * STAGE_BYTES;
@@ -178,9 +205,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   } else if (warp == 1) {
     if (lane == 0 && leader) {
       uint32_t stage = 0, phase = 0, acc = 0, acc_phase = 0;
-      for (int item = worker; item < n_items; item += n_workers) {
-        const int split = item % p.splits;
-        const int kb0 = split * kb_per, kb1 = min(kb0 + kb_per, p.kb_total);
+      Work work = work0;
+      for (int tile, kb0, kb1; work.next(tile, kb0, kb1);) {
         mbar_wait(&tempty[acc], acc_phase ^ 1, 2);      // epilogue (of both CTAs) has drained this accumulator
         tc_fence_after();
         const uint32_t tmem_d = tmem_base + acc * BLOCK_N;
@@ -216,8 +242,8 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
     uint8_t* my_stage = staging + (warp - 2) * (EPI_BUFS * 4096);
     float* my_bias = bias_s + (warp - 2) * BLOCK_N;
     uint32_t acc = 0, acc_phase = 0, sbuf = 0;
-    for (int item = worker; item < n_items; item += n_workers) {
-      const int tile = item / p.splits;
+    Work work = work0;
+    for (int tile, kb0, kb1; work.next(tile, kb0, kb1);) {
       const int m0 = (tile % p.tiles_m) * (BLOCK_M * CG) + (int)rank * BLOCK_M, n0 = (tile / p.tiles_m) * BLOCK_N;
       if (!ACCUM) {                                   // bias slice of this tile, fetched under the main loop
 #pragma unroll
@@ -470,11 +496,25 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
     }
   }
   p.splits = splits;
+  p.range_mode = 0;
+  if (out_f32_accum && getenv("PACI_GEMM_RANGE") == nullptr) {
+    // equal contiguous (tile, k-block) ranges instead of whole items: U / W k-blocks per worker plus one flush per
+    // tile boundary crossed (+1).  Taken for outputs of many rounds (the LM-head wgrad: 788 tiles, 10.65 rounds ->
+    // 0.659 to 0.601 ms); with fewer tiles than two rounds the k-block rate itself drops when every pair is busy
+    // (the operand stream is near the L2 bandwidth: 64 KB per 512 MMA cycles per pair), and the round-robin splits
+    // measured the same or better
+    const int EPI = 8;
+    const long units = (long)tiles * p.kb_total;
+    const long per = ceil_div(units, (long)workers);
+    const long cost = per + (ceil_div(per, (long)p.kb_total) + 1) * EPI;
+    const long item_cost = ceil_div((long)tiles * splits, (long)workers) * (ceil_div(p.kb_total, splits) + EPI);
+    if (tiles >= 2 * workers && cost < item_cost) p.range_mode = 1;
+  }
   // balanced persistent grid: the same number of rounds on the fewest workers (128 tiles on 74 pairs take 2
   // rounds; so do 64 pairs, and the other 20 SMs stay free for the other stage streams' kernels)
   const int items = tiles * splits;
   const int rounds = ceil_div(items, workers);
-  const int grid = ceil_div(items, rounds) * CG;
+  const int grid = (p.range_mode ? workers : ceil_div(items, rounds)) * CG;
 #define GO(CG_, BN_, ST_, AMN, BMN, ACC) return launch<CG_, BN_, ST_, AMN, BMN, ACC>(tmA, tmB, tmC, tmC2, p, grid, s)
 #define BY_LAYOUT(CG_, BN_, ST_)                                                                          \
   do {                                                                                                    \
