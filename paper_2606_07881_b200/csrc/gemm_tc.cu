@@ -500,9 +500,8 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
   if (out_f32_accum && getenv("PACI_GEMM_RANGE") == nullptr) {
     // equal contiguous (tile, k-block) ranges instead of whole items: U / W k-blocks per worker plus one flush per
     // tile boundary crossed (+1).  Taken for outputs of many rounds (the LM-head wgrad: 788 tiles, 10.65 rounds ->
-    // 0.659 to 0.601 ms); with fewer tiles than two rounds the k-block rate itself drops when every pair is busy
-    // (the operand stream is near the L2 bandwidth: 64 KB per 512 MMA cycles per pair), and the round-robin splits
-    // measured the same or better
+    // 0.659 to 0.597 ms); with fewer tiles than two rounds the k-block rate itself drops when every pair is busy
+    // and the round-robin splits measured the same or better
     const int EPI = 8;
     const long units = (long)tiles * p.kb_total;
     const long per = ceil_div(units, (long)workers);
