@@ -185,3 +185,31 @@ def test_layernorm_pipelined_kernels_full_size(rows, with_res):
     assert rel_l2(host(Gb) + 0.25, db_ref) < TOL[pb.BF16] / 4
     if with_res:
         assert rel_l2(host(Gc) - 1.0, host(dx).astype(np.float64).sum(0)) < 1e-4
+
+
+def test_eight_stage_streams_full_width_counts():
+    """configs[3]'s concurrency at full width: 8 emulated stages (one block each, D 1024, H 16, T 1024, micro-batch 8,
+    k = 2) on 8 streams, 24 micro-batches.  The oracle's model is out of reach at this size, so the unique results
+    are compared -- crossed updates (Eq. 8), versions and admission maxima against the oracle's event simulator,
+    exactly -- and the rest is checked for validity: every loss finite and below 2 ln V (the first sign-like AdamW
+    steps of eight stale stages overshoot for a few micro-batches), the last losses below the first.  Barrier waits
+    trap after 4 s, so a protocol error under 8-stream concurrency fails here instead of hanging the GPU.  (This run
+    is too short to reproduce the ring-phase hang that `bench.py --config medium8` once showed: that one is closed
+    by construction, a static_assert on the stage / warp-set counts of the LayerNorm ring.)"""
+    from oracle import schedule
+    from test_gpu_pipeline import _build
+    S, L, mu, k, n, Vs, lr = 8, 1, MU, 2, 24, 2048, 3e-4
+    _, _, stages = _build(pb.BF16, S, L, D, H, T, mu, Vs, k, seed=11)
+    tok = synth.tokens(11, n, mu, T, Vs, "zipf")
+    out = pb.Pipeline(stages).run(torch.from_numpy(tok).cuda(), lr)
+    ref = schedule.simulate(S, n, k)
+    assert out["delta"].tolist() == ref["delta"]
+    assert out["version"].tolist() == ref["version"]
+    assert out["max_q"].tolist() == ref["max_q"]
+    for s in range(S):
+        assert max(ref["delta"][s]) <= schedule.delta_bound(S, s + 1, k)
+    loss = out["loss"]
+    assert np.all(np.isfinite(loss)) and loss.max() < 2 * np.log(Vs)
+    assert loss[-4:].mean() < loss[:4].mean()
+    for st in stages:
+        st.close()
