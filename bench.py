@@ -381,7 +381,7 @@ def run_ours(args, c, name):
                        "stage_steps_per_step": S * n_micro,
                        "l2": "inputs larger than L2 (each step streams > 20 GB of weights and stashed activations)",
                        "parallelism": "replicas only" if world > 1 else "1 GPU, S emulated stages on per-stage streams",
-                       "gemm_backend": "tcgen05" if pb.lib.paci_gemm_backend_is_tcgen05() else "simt"},
+                       "gemm_backend": "tcgen05"},
             "pipeline_tokens_per_s": value / S, "wall_ms_per_step": wall_ms / args.steps,
             "sampled_region_ms_per_step": prof_ms / args.steps,
             "clocks": clk,

@@ -27,6 +27,8 @@
  *   - activations are row-major [mu, T, D] in the stage's compute dtype (float for PACI_FP32,
  *     __nv_bfloat16 for PACI_BF16); tokens/targets are int32 [mu, T].
  *   - stage_index s is 0-based; the paper's stage i is s+1, its N is n_stages, its a is k_accum.
+ *   - one kernel family per dtype (PACI_FP32: FFMA parity kernels; PACI_BF16: tcgen05 / TMA kernels); no
+ *     environment switches, no fallback paths.
  */
 #ifndef PACI_H_
 #define PACI_H_
@@ -68,7 +70,7 @@ typedef struct paci_stage_config {
   int32_t n_layers;      /* pre-LN GPT-2 decoder blocks on this stage (>= 0)                      */
   int32_t d_model;       /* D, multiple of 8 (bf16: multiple of 64)                                */
   int32_t n_heads;       /* H, D % H == 0; head dim 64 in PACI_BF16, any <= 128 in PACI_FP32      */
-  int32_t seq_len;       /* T                                                                      */
+  int32_t seq_len;       /* T (bf16: multiple of 128)                                              */
   int32_t micro_batch;   /* mu sequences per micro-batch; M = mu*T tokens                          */
   int32_t k_accum;       /* k (paper a): local backwards per optimizer update                      */
   int32_t vocab;         /* V (used when has_embedding or has_head)                                */
@@ -78,6 +80,17 @@ typedef struct paci_stage_config {
                          /* gradient); otherwise the stage owns its own copy "head.w" (DESIGN R10)  */
   int32_t dtype;         /* PACI_FP32 | PACI_BF16                                                  */
   float beta1, beta2, eps, weight_decay;   /* AdamW: 0.9, 0.95, 1e-8, 0.1 in the paper    */
+  int32_t checkpoint;    /* 0: backward differentiates the activations STASHED at forward time and  */
+                         /*    evaluates them at the current parameters (Eq. 1).              */
+                         /* 1: activation-checkpointed PACI (App. B "Activation checkpointing",     */
+                         /*    P:282): only the stage INPUT (tokens / h, and the targets) is kept;  */
+                         /*    backward first recomputes the stage forward under the stage's        */
+                         /*    CURRENT parameter version, then differentiates that.  Same single    */
+                         /*    parameter copy; a stash slot shrinks to the stage input.             */
+  float   dropout_p;     /* dropout probability (0.1) on the embedding output and on the     */
+                         /* output of both residual branches of every block (R23); 0 = off */
+  uint64_t dropout_seed; /* key of the counter-based mask generator (Philox4x32-10, counter =       */
+                         /* (mb_id, site, element/4)); backward regenerates the forward's mask      */
 } paci_stage_config;
 
 /* Bytes of DEVICE workspace a stage with this config needs (parameters, m, v, G, bf16 shadow,
@@ -115,6 +128,13 @@ int paci_stage_read(paci_stage_t* st, int what, const char* name, float* host_ds
  * stash slot, q_s += 1. */
 int paci_forward(paci_stage_t* st, int64_t mb_id, const void* in, const int32_t* targets, void* out,
                  void* stream);
+/* The same with n_seq <= micro_batch sequences in this micro-batch (heterogeneous micro-batch sizes,
+ * App. B "Micro-batching": "the first B mod m micro-batches contain floor(B/m)+1 sequences and the
+ * remaining micro-batches contain floor(B/m) sequences").  in / targets / out hold n_seq sequences; the loss
+ * is the mean over the n_seq*T tokens of THIS micro-batch (R22).  paci_backward of mb_id works on
+ * the n_seq recorded here. */
+int paci_forward_var(paci_stage_t* st, int64_t mb_id, int32_t n_seq, const void* in, const int32_t* targets,
+                     void* out, void* stream);
 
 /* Backward of micro-batch mb_id (Alg. 1 lines 11-15): must be the oldest unresolved forward.
  *   dout DEVICE: grad wrt the stage output [mu,T,D] (compute dtype); NULL iff has_head
@@ -128,6 +148,24 @@ int paci_backward(paci_stage_t* st, int64_t mb_id, const void* dout, void* din, 
  * version += 1, c_s = 0.  Returns 1 if it stepped, 0 if not yet, < 0 on error.  This is the only
  * call that changes parameters. */
 int paci_maybe_step(paci_stage_t* st, float lr, void* stream);
+
+/* Learning-rate schedule of App. B: linear warm-up over warmup_steps updates to `peak`, then cosine
+ * decay to final_frac * peak at total_steps (paper: 1% warm-up, final_frac 0.1).  `step` = the stage's local
+ * update index t (paci_version) BEFORE the update it is used for.  Pure host arithmetic (no device work):
+ *   step <  warmup : peak * (step + 1) / warmup
+ *   else           : peak * (f + (1 - f) * 0.5 * (1 + cos(pi * (step - warmup) / (total - warmup)))), clamped at
+ *                    step >= total to peak * f.                                              (R16) */
+float paci_lr_schedule(int64_t step, int64_t total_steps, int64_t warmup_steps, float peak, float final_frac);
+
+/* Checkpoint / resume of the counters that paci_stage_load cannot reach: sets the local update index t
+ * (also the AdamW bias-correction step and the DEVICE version word) and the window count c (0 <= c < k; the
+ * matching partial sum must have been loaded into PACI_GRAD_ACCUM).  Only legal with no unresolved forward
+ * (q = 0), else PACI_ESTATE.  Synchronises `stream`. */
+int paci_stage_set_state(paci_stage_t* st, int64_t version, int32_t window_count, void* stream);
+/* Device-side input validation: token / target ids outside [0, vocab) are CLAMPED by the kernels (never an
+ * out-of-bounds access) and raise a sticky device flag.  Synchronises `stream`; returns PACI_EINVAL if the
+ * flag is set (and clears it), else PACI_OK. */
+int paci_stage_check(paci_stage_t* st, void* stream);
 
 int64_t paci_version(const paci_stage_t* st);          /* local updates applied so far (t)       */
 int32_t paci_unresolved(const paci_stage_t* st);       /* q_s                                          */
@@ -175,7 +213,19 @@ int paci_pipeline_destroy(paci_pipeline_t* p);
  *           issued at a stage before that stage applied update g.
  * Blocks until the run is complete. */
 int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_on_host,
-                      int64_t n_microbatches, int32_t mode, float lr, paci_run_report* rep);
+                      int64_t n_microbatches, int32_t mode, float lr, void* stream, paci_run_report* rep);
+/* `stream` (both calls): the CALLER's stream.  The run is ordered after everything already enqueued on it (the
+ * producer of a DEVICE token buffer, a non-blocking copy from pinned memory); NULL = the legacy default stream.
+ * The stage streams are the pipeline's own.  Token ids are validated on the device: PACI_EINVAL after the run if
+ * any id was outside [0, vocab) (the kernels clamp, so no access is out of bounds).
+ *
+ * paci_pipeline_run_var: heterogeneous micro-batch sizes.  n_seq: HOST int32 [n_microbatches], each in
+ * [1, micro_batch] (NULL = all micro_batch); micro-batch m uses the first n_seq[m] sequences of tokens[m].
+ * lr_by_update: HOST float [n_updates] or NULL: learning rate of a stage's u-th update DURING THIS RUN (u =
+ * version - version at the start of the run), e.g. filled from paci_lr_schedule; NULL = constant lr. */
+int paci_pipeline_run_var(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_on_host,
+                          int64_t n_microbatches, const int32_t* n_seq, int32_t mode, float lr,
+                          const float* lr_by_update, int64_t n_updates, void* stream, paci_run_report* rep);
 
 /* ---- op-level entry points (kernel parity tests and per-kernel roofline measurements) ------ */
 /* All pointers DEVICE.  dtype = PACI_FP32 | PACI_BF16 selects the activation type T below. */
@@ -217,12 +267,18 @@ int paci_op_attention_fwd(int dtype, int mu, int T, int H, int dh, const void* q
 int paci_op_attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
                           const void* o, const float* lse, void* dqkv, float* scratch, void* stream);
 size_t paci_op_attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh);
-/* x = wte[tok] + wpe[pos] (a1);  tok int32 [mu,T]; wte, wpe fp32. */
-int paci_op_embed_fwd(int dtype, int mu, int T, int D, const int32_t* tok, const float* wte,
+/* x = wte[tok] + wpe[pos] (a1);  tok int32 [mu,T]; wte [vocab, D], wpe fp32.  Ids outside [0, vocab) are clamped. */
+int paci_op_embed_fwd(int dtype, int mu, int T, int D, int vocab, const int32_t* tok, const float* wte,
                       const float* wpe, void* x, void* stream);
 /* Gwte[tok] += dx;  Gwpe[t] += sum_b dx  (a19). */
-int paci_op_embed_bwd(int dtype, int mu, int T, int D, const int32_t* tok, const void* dx, float* Gwte,
+int paci_op_embed_bwd(int dtype, int mu, int T, int D, int vocab, const int32_t* tok, const void* dx, float* Gwte,
                       float* Gwpe, void* stream);
+/* Dropout with the counter-based mask of paci_stage_config.dropout_seed: element e of x (n elements, T) is
+ * kept iff word e % 4 of Philox4x32-10(counter = (e/4 lo, e/4 hi, (uint32) mb_id, site), key = (seed lo, seed hi))
+ * is >= floor(p 2^32); kept values are multiplied by 1/(1-p).  out may alias x.  Forward and backward apply the
+ * same map. */
+int paci_op_dropout(int dtype, size_t n, const void* x, void* out, float p, uint64_t seed, int64_t mb_id,
+                    int32_t site, void* stream);
 /* loss[0] += sum_rows (lse - z[tgt]) / rows;  z <- dz = (softmax(z) - onehot) / rows in place.
  * z is [rows, ldz] with V valid columns (padding columns are written 0).  (a11) */
 int paci_op_softmax_ce(int dtype, int rows, int V, int ldz, void* z, const int32_t* tgt, float* loss,
@@ -251,9 +307,9 @@ const char* paci_profile_category_name(int32_t cat);
 
 /* Number of kernels the library has launched in this process (for bench.py's gpu_launches). */
 int64_t paci_launch_count(void);
-/* 1 if the tcgen05 GEMM path is in use for PACI_BF16 GEMMs, 0 if the SIMT fallback was forced by
- * the environment variable PACI_GEMM=simt (a debugging aid, never a silent fallback). */
-int paci_gemm_backend_is_tcgen05(void);
+/* Work decomposition the LAST PACI_BF16 GEMM launched from this thread took (tests assert the path they
+ * mean to cover): out6 = {cta_group, block_n, splits, range_mode, grid, tiles}.  HOST int32 [6]. */
+void paci_gemm_last_plan(int32_t* out6);
 
 #ifdef __cplusplus
 }

@@ -24,10 +24,21 @@ as rows [q; k; v] with head h = rows h*dh..(h+1)*dh-1, weights stored [out, in],
 
 Everything is float64 numpy.  A library matmul (`@`) serves as the contraction step; there is
 no blocking, fusion or reordering beyond the formulas written here.
+
+Two optional extensions, both off by default so that everything above is unchanged:
+
+* `drop=(p, seed, mb_id)`: dropout ("dropout to 0.1") on the embedding output and on the output of both
+  residual branches of every block (R23), mask from `oracle.dropout` (a pure function of seed,
+  micro-batch id, site and element index);
+* `stage_backward_checkpointed`: activation-checkpointed PACI (App. B): "discarded activations can be
+  recomputed during the backward pass using the stage's current parameter version ... With checkpointing, those
+  activations are instead recomputed under the current parameter version before differentiation."
 """
 from __future__ import annotations
 
 import numpy as np
+
+from . import dropout as _dropout
 
 LN_EPS = 1e-5                      # DESIGN.md R13
 GELU_C = np.sqrt(2.0 / np.pi)      # DESIGN.md R12 (tanh form)
@@ -158,29 +169,46 @@ def cross_entropy_fwd_bwd(z, tgt):
 
 # ----------------------------------------------------------------------------- block
 
-def block_fwd(x, P, pre, H):
-    """x1 = x + Attn(LN1(x));  x2 = x1 + MLP(LN2(x1))."""
+def _mask(drop, shape, site):
+    """drop = (p, seed, mb_id) or None -> multiplicative mask (1/(1-p) kept, 0 dropped) or None."""
+    if drop is None or drop[0] <= 0.0:
+        return None
+    p, seed, mb_id = drop
+    return _dropout.mask(shape, p, seed, mb_id, site)
+
+
+def block_fwd(x, P, pre, H, drop=None, l=0):
+    """x1 = x + drop(Attn(LN1(x)));  x2 = x1 + drop(MLP(LN2(x1)))   (drop = identity unless `drop` is given)."""
     y1, st_ln1 = layernorm_fwd(x, P[pre + "ln1.g"], P[pre + "ln1.b"])
     qkv, st_qkv = linear_fwd(y1, P[pre + "attn.wqkv"], P[pre + "attn.bqkv"])
     o, st_att = attention_fwd(qkv, H)
     a, st_o = linear_fwd(o, P[pre + "attn.wo"], P[pre + "attn.bo"])
+    mask_a = _mask(drop, a.shape, _dropout.site_attn(l))
+    if mask_a is not None:
+        a = a * mask_a
     x1 = x + a
     y2, st_ln2 = layernorm_fwd(x1, P[pre + "ln2.g"], P[pre + "ln2.b"])
     p, st_w1 = linear_fwd(y2, P[pre + "mlp.w1"], P[pre + "mlp.b1"])
     g = gelu_fwd(p)
     m, st_w2 = linear_fwd(g, P[pre + "mlp.w2"], P[pre + "mlp.b2"])
+    mask_m = _mask(drop, m.shape, _dropout.site_mlp(l))
+    if mask_m is not None:
+        m = m * mask_m
     x2 = x1 + m
-    return x2, dict(ln1=st_ln1, qkv=st_qkv, att=st_att, o=st_o, ln2=st_ln2, w1=st_w1, p=p, w2=st_w2)
+    return x2, dict(ln1=st_ln1, qkv=st_qkv, att=st_att, o=st_o, ln2=st_ln2, w1=st_w1, p=p, w2=st_w2,
+                    mask_a=mask_a, mask_m=mask_m)
 
 
 def block_bwd(dx2, st, Pc, pre, grads):
     """Backward of block_fwd with stash `st` and CURRENT parameters `Pc`; adds into `grads`."""
-    dg, dW2, db2 = linear_bwd(dx2, st["w2"], Pc[pre + "mlp.w2"])
+    dm = dx2 if st.get("mask_m") is None else dx2 * st["mask_m"]          # grad wrt the MLP branch output
+    dg, dW2, db2 = linear_bwd(dm, st["w2"], Pc[pre + "mlp.w2"])
     dp = gelu_bwd(dg, st["p"])
     dy2, dW1, db1 = linear_bwd(dp, st["w1"], Pc[pre + "mlp.w1"])
     dln2, dg2, dbt2 = layernorm_bwd(dy2, st["ln2"], Pc[pre + "ln2.g"])
     dx1 = dx2 + dln2
-    do, dWo, dbo = linear_bwd(dx1, st["o"], Pc[pre + "attn.wo"])
+    da = dx1 if st.get("mask_a") is None else dx1 * st["mask_a"]          # grad wrt the attention branch output
+    do, dWo, dbo = linear_bwd(da, st["o"], Pc[pre + "attn.wo"])
     dqkv = attention_bwd(do, st["att"])
     dy1, dWqkv, dbqkv = linear_bwd(dqkv, st["qkv"], Pc[pre + "attn.wqkv"])
     dln1, dg1, dbt1 = layernorm_bwd(dy1, st["ln1"], Pc[pre + "ln1.g"])
@@ -209,22 +237,27 @@ class StageSpec:
         return "wte" if self.has_embedding else "head.w"
 
 
-def stage_forward(spec, P, inp, targets=None):
+def stage_forward(spec, P, inp, targets=None, drop=None):
     """h_{m,i} = F_i(h_{m,i-1}; theta_i)  (Eq. 7, P:382).
 
     inp: int tokens [mu,T] on the first stage, else h [mu,T,D].  Returns (out, stash) where out is
     h [mu,T,D], or the scalar loss on the last stage (then `targets` [mu,T] is required).
     `stash` = "activations required for backpropagation" (Alg. 1 line 7).
+    mu is read off `inp`: a micro-batch may hold fewer sequences than spec.micro_batch, and the loss is
+    the mean over the tokens of THIS micro-batch (R22).  drop = (p, seed, mb_id) switches dropout on.
     """
     st = {}
     if spec.has_embedding:
         st["tok"] = inp
         x = embed_fwd(inp, P["wte"], P["wpe"])
+        st["mask_e"] = _mask(drop, x.shape, _dropout.SITE_EMBED)
+        if st["mask_e"] is not None:
+            x = x * st["mask_e"]
     else:
         x = inp
     st["blocks"] = []
     for l in range(spec.n_layers):
-        x, sb = block_fwd(x, P, f"h.{l}.", spec.n_heads)
+        x, sb = block_fwd(x, P, f"h.{l}.", spec.n_heads, drop, l)
         st["blocks"].append(sb)
     if not spec.has_head:
         return x, st
@@ -250,8 +283,23 @@ def stage_backward(spec, Pc, stash, dout=None):
     for l in reversed(range(spec.n_layers)):
         dx = block_bwd(dx, stash["blocks"][l], Pc, f"h.{l}.", grads)
     if spec.has_embedding:
+        if stash.get("mask_e") is not None:
+            dx = dx * stash["mask_e"]
         dwte, dwpe = embed_bwd(dx, stash["tok"], spec.vocab)
         grads["wte"] = grads.get("wte", 0.0) + dwte
         grads["wpe"] = dwpe
         return None, grads
     return dx, grads
+
+
+def stage_backward_checkpointed(spec, Pc, stage_input, targets=None, dout=None, drop=None):
+    """Activation-checkpointed PACI (App. B): nothing but the stage INPUT was kept at forward time; the
+    activations "are instead recomputed under the current parameter version before differentiation".
+
+    So: re-run F_i on the stashed input with the CURRENT parameters Pc (same dropout mask: it is a function of
+    the micro-batch id), then differentiate that recomputation at Pc.  The incoming `dout` was produced by the
+    ORIGINAL pipeline computation -- that is the mismatch the paper describes.  Identical to `stage_backward` of
+    the stashed forward iff no update fell between forward and backward (Delta = 0).
+    """
+    _, stash = stage_forward(spec, Pc, stage_input, targets, drop)
+    return stage_backward(spec, Pc, stash, dout)

@@ -13,9 +13,18 @@ from . import model, schedule
 from .adamw import StageOptimizer
 
 
-def run_pipeline(specs, params, tokens, k, lr, mode="paci", m_f=None, sim_kwargs=None, hyper=None):
+def run_pipeline(specs, params, tokens, k, lr, mode="paci", m_f=None, sim_kwargs=None, hyper=None,
+                 checkpoint=False, n_seq=None, dropout=None, lr_by_update=None):
     """specs: list of model.StageSpec (one per stage); params: list of dict name->array;
     tokens: int [n_mb, mu, T+1] (targets are tokens shifted by one).
+
+    Optional:
+      checkpoint    activation-checkpointed PACI: a stage keeps only its input and recomputes its forward
+                    under the CURRENT parameters at backward time (model.stage_backward_checkpointed);
+      n_seq         int [n_mb]: micro-batch m holds only the first n_seq[m] sequences of tokens[m] (heterogeneous
+                    micro-batch sizes, P:274);
+      dropout       (p, seed): dropout with the counter-based mask of oracle.dropout, keyed by the micro-batch id;
+      lr_by_update  list: learning rate of a stage's u-th update (each stage indexes it by its own update count).
 
     Returns dict(losses[n_mb], delta[s][m], version[s], opt[s] (StageOptimizer: theta, m, v, G),
                  sim (the schedule record)).
@@ -33,11 +42,14 @@ def run_pipeline(specs, params, tokens, k, lr, mode="paci", m_f=None, sim_kwargs
     vF = [[None] * n_mb for _ in range(S)]
     for (_, _, s, kind, m) in sim["ops"]:
         spec = specs[s]
+        ns = tokens.shape[1] if n_seq is None else int(n_seq[m])
+        drop = None if dropout is None else (dropout[0], dropout[1], m)
         if kind == "F":
-            inp = tokens[m, :, :-1].astype(np.int64) if s == 0 else h[s].pop(m)
-            tgt = tokens[m, :, 1:].astype(np.int64) if spec.has_head else None
+            inp = tokens[m, :ns, :-1].astype(np.int64) if s == 0 else h[s].pop(m)
+            tgt = tokens[m, :ns, 1:].astype(np.int64) if spec.has_head else None
             vF[s][m] = opt[s].version
-            out, stash[s][m] = model.stage_forward(spec, opt[s].theta, inp, tgt)
+            out, st = model.stage_forward(spec, opt[s].theta, inp, tgt, drop)
+            stash[s][m] = (inp, tgt) if checkpoint else st          # checkpoint: the stage input is all that is kept
             if spec.has_head:
                 losses[m] = out
             else:
@@ -45,12 +57,17 @@ def run_pipeline(specs, params, tokens, k, lr, mode="paci", m_f=None, sim_kwargs
         elif kind == "B":
             dout = None if spec.has_head else dh[s].pop(m)
             delta[s][m] = opt[s].version - vF[s][m]
-            din, grads = model.stage_backward(spec, opt[s].theta, stash[s].pop(m), dout)
+            if checkpoint:
+                inp, tgt = stash[s].pop(m)
+                din, grads = model.stage_backward_checkpointed(spec, opt[s].theta, inp, tgt, dout, drop)
+            else:
+                din, grads = model.stage_backward(spec, opt[s].theta, stash[s].pop(m), dout)
             opt[s].accumulate(grads)
             if s > 0:
                 dh[s - 1][m] = din
         else:  # "U"
-            stepped = opt[s].maybe_step(lr)
+            lr_now = lr if lr_by_update is None else lr_by_update[opt[s].version]
+            stepped = opt[s].maybe_step(lr_now)
             assert stepped and opt[s].version == m
     assert delta == sim["delta"]
     return dict(losses=losses, delta=delta, version=[o.version for o in opt], opt=opt, sim=sim)

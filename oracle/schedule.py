@@ -41,6 +41,11 @@ def eta_flush(m: int, n_stages: int) -> float:
     return m / (m + n_stages - 1)
 
 
+def eta_inter(m: int, n_stages: int, v: int) -> float:
+    """Eq. 4: interleaved 1F1B with V virtual stages per device, eta = m V / (m V + N - 1)."""
+    return m * v / (m * v + n_stages - 1)
+
+
 def simulate(S, n_mb, k, tF=None, tB=None, tU=None, lat=0, mode="paci", m_f=None,
              backward_first=True):
     """Run Alg. 1 on S stages for n_mb micro-batches.  Returns a dict:

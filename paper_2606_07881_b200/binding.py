@@ -25,7 +25,8 @@ class StageConfig(C.Structure):
     _fields_ = [(n, C.c_int32) for n in (
         "stage_index", "n_stages", "n_layers", "d_model", "n_heads", "seq_len", "micro_batch", "k_accum",
         "vocab", "has_embedding", "has_head", "dtype")] + [(n, C.c_float) for n in (
-            "beta1", "beta2", "eps", "weight_decay")]
+            "beta1", "beta2", "eps", "weight_decay")] + [
+        ("checkpoint", C.c_int32), ("dropout_p", C.c_float), ("dropout_seed", C.c_uint64)]
 
 
 class RunReport(C.Structure):
@@ -52,8 +53,12 @@ SIGNATURES = {
     "paci_stage_load": (_i, [_vp, _i, C.c_char_p, _vp, _sz, _vp]),
     "paci_stage_read": (_i, [_vp, _i, C.c_char_p, _vp, _sz, _vp]),
     "paci_forward": (_i, [_vp, _i64, _vp, _vp, _vp, _vp]),
+    "paci_forward_var": (_i, [_vp, _i64, C.c_int32, _vp, _vp, _vp, _vp]),
     "paci_backward": (_i, [_vp, _i64, _vp, _vp, _vp]),
     "paci_maybe_step": (_i, [_vp, _f, _vp]),
+    "paci_lr_schedule": (_f, [_i64, _i64, _i64, _f, _f]),
+    "paci_stage_set_state": (_i, [_vp, _i64, C.c_int32, _vp]),
+    "paci_stage_check": (_i, [_vp, _vp]),
     "paci_version": (_i64, [_vp]),
     "paci_unresolved": (C.c_int32, [_vp]),
     "paci_window_count": (C.c_int32, [_vp]),
@@ -63,7 +68,9 @@ SIGNATURES = {
     "paci_pipeline_workspace_bytes": (_sz, [C.POINTER(_vp), C.c_int32]),
     "paci_pipeline_create": (_i, [C.POINTER(_vp), C.c_int32, _vp, _sz, C.POINTER(_vp)]),
     "paci_pipeline_destroy": (_i, [_vp]),
-    "paci_pipeline_run": (_i, [_vp, _vp, C.c_int32, _i64, C.c_int32, _f, C.POINTER(RunReport)]),
+    "paci_pipeline_run": (_i, [_vp, _vp, C.c_int32, _i64, C.c_int32, _f, _vp, C.POINTER(RunReport)]),
+    "paci_pipeline_run_var": (_i, [_vp, _vp, C.c_int32, _i64, _vp, C.c_int32, _f, _vp, _i64, _vp,
+                                   C.POINTER(RunReport)]),
     "paci_op_gemm": (_i, [_i, _i, _i, _i, _i, _vp, _i, _vp, _i, _vp, _vp, _i, _i, _vp]),
     "paci_op_gemm_bias_gelu": (_i, [_i, _i, _i, _i, _vp, _i, _vp, _i, _vp, _vp, _vp, _i, _vp]),
     "paci_op_layernorm_fwd": (_i, [_i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -74,15 +81,16 @@ SIGNATURES = {
     "paci_op_attention_fwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp]),
     "paci_op_attention_bwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_attention_bwd_scratch_bytes": (_sz, [_i, _i, _i, _i, _i]),
-    "paci_op_embed_fwd": (_i, [_i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
-    "paci_op_embed_bwd": (_i, [_i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
+    "paci_op_embed_fwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
+    "paci_op_embed_bwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
+    "paci_op_dropout": (_i, [_i, _sz, _vp, _vp, _f, C.c_uint64, _i64, C.c_int32, _vp]),
     "paci_op_softmax_ce": (_i, [_i, _i, _i, _i, _vp, _vp, _vp, _vp]),
     "paci_op_adamw": (_i, [_sz, _sz, _vp, _vp, _vp, _vp, _vp, _i, _i64, _f, _f, _f, _f, _f, _vp, _vp]),
     "paci_profile_begin": (_i, [C.c_int32]),
     "paci_profile_end": (_i, [C.POINTER(ProfEntry)]),
     "paci_profile_category_name": (C.c_char_p, [C.c_int32]),
     "paci_launch_count": (_i64, []),
-    "paci_gemm_backend_is_tcgen05": (_i, []),
+    "paci_gemm_last_plan": (None, [C.POINTER(C.c_int32)]),
 }
 
 
@@ -131,12 +139,23 @@ def _stream(stream=None):
 
 
 def make_config(stage_index, n_stages, n_layers, d_model, n_heads, seq_len, micro_batch, k_accum, vocab,
-                dtype, has_embedding=None, has_head=None, beta1=0.9, beta2=0.95, eps=1e-8, weight_decay=0.1):
+                dtype, has_embedding=None, has_head=None, beta1=0.9, beta2=0.95, eps=1e-8, weight_decay=0.1,
+                checkpoint=0, dropout_p=0.0, dropout_seed=0):
     """AdamW defaults are the paper's."""
     return StageConfig(stage_index, n_stages, n_layers, d_model, n_heads, seq_len, micro_batch, k_accum, vocab,
                        int(stage_index == 0 if has_embedding is None else has_embedding),
                        int(stage_index == n_stages - 1 if has_head is None else has_head),
-                       dtype, beta1, beta2, eps, weight_decay)
+                       dtype, beta1, beta2, eps, weight_decay, int(checkpoint), float(dropout_p), int(dropout_seed))
+
+
+def gemm_last_plan() -> dict:
+    out = (C.c_int32 * 6)()
+    lib.paci_gemm_last_plan(out)
+    return dict(zip(("cta_group", "block_n", "splits", "range_mode", "grid", "tiles"), list(out)))
+
+
+def lr_schedule(step, total_steps, warmup_steps, peak, final_frac=0.1) -> float:
+    return float(lib.paci_lr_schedule(step, total_steps, warmup_steps, peak, final_frac))
 
 
 class Stage:
@@ -165,13 +184,18 @@ class Stage:
 
     __del__ = close
 
+    def _dev(self):
+        import torch
+        return torch.cuda.device(self.device)
+
     def numel(self, name):
         return lib.paci_stage_tensor_numel(self.handle, name.encode())
 
     def load(self, name, array, what=PARAM):
         a = np.ascontiguousarray(array, dtype=np.float32)
-        check(lib.paci_stage_load(self.handle, what, name.encode(), a.ctypes.data, a.size, _stream()),
-              f"paci_stage_load({name})")
+        with self._dev():
+            check(lib.paci_stage_load(self.handle, what, name.encode(), a.ctypes.data, a.size, _stream()),
+                  f"paci_stage_load({name})")
 
     def load_params(self, params: dict):
         for n, a in params.items():
@@ -182,21 +206,38 @@ class Stage:
         if n == 0:
             raise KeyError(name)
         out = np.empty(n, dtype=np.float32)
-        check(lib.paci_stage_read(self.handle, what, name.encode(), out.ctypes.data, n, _stream()),
-              f"paci_stage_read({name})")
+        with self._dev():
+            check(lib.paci_stage_read(self.handle, what, name.encode(), out.ctypes.data, n, _stream()),
+                  f"paci_stage_read({name})")
         return out.reshape(shape) if shape is not None else out
 
-    def forward(self, mb_id, inp, targets=None, out=None, stream=None, raise_on_again=True):
-        rc = lib.paci_forward(self.handle, mb_id, _ptr(inp), _ptr(targets), _ptr(out), _stream(stream))
+    def forward(self, mb_id, inp, targets=None, out=None, stream=None, raise_on_again=True, n_seq=None):
+        with self._dev():
+            if n_seq is None:
+                rc = lib.paci_forward(self.handle, mb_id, _ptr(inp), _ptr(targets), _ptr(out), _stream(stream))
+            else:
+                rc = lib.paci_forward_var(self.handle, mb_id, n_seq, _ptr(inp), _ptr(targets), _ptr(out),
+                                          _stream(stream))
         if rc == EAGAIN and not raise_on_again:
             return rc
         return check(rc, "paci_forward")
 
     def backward(self, mb_id, dout=None, din=None, stream=None):
-        return check(lib.paci_backward(self.handle, mb_id, _ptr(dout), _ptr(din), _stream(stream)), "paci_backward")
+        with self._dev():
+            return check(lib.paci_backward(self.handle, mb_id, _ptr(dout), _ptr(din), _stream(stream)),
+                         "paci_backward")
 
     def maybe_step(self, lr, stream=None):
-        return check(lib.paci_maybe_step(self.handle, lr, _stream(stream)), "paci_maybe_step")
+        with self._dev():
+            return check(lib.paci_maybe_step(self.handle, lr, _stream(stream)), "paci_maybe_step")
+
+    def set_state(self, version, window_count):
+        with self._dev():
+            check(lib.paci_stage_set_state(self.handle, version, window_count, _stream()), "paci_stage_set_state")
+
+    def check_inputs(self):
+        with self._dev():
+            check(lib.paci_stage_check(self.handle, _stream()), "paci_stage_check")
 
     @property
     def version(self):
@@ -215,8 +256,9 @@ class Stage:
 
     def device_stamps(self, mb_id):
         vF, vB = C.c_int64(), C.c_int64()
-        check(lib.paci_stage_device_stamps(self.handle, mb_id, C.byref(vF), C.byref(vB), _stream()),
-              "paci_stage_device_stamps")
+        with self._dev():
+            check(lib.paci_stage_device_stamps(self.handle, mb_id, C.byref(vF), C.byref(vB), _stream()),
+                  "paci_stage_device_stamps")
         return vF.value, vB.value
 
 
@@ -232,10 +274,12 @@ class Pipeline:
         nbytes = lib.paci_pipeline_workspace_bytes(arr, S)
         if nbytes == 0:
             raise PaciError(EINVAL, "paci_pipeline_workspace_bytes")
-        self.ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.stages[0].device)
+        self.device = self.stages[0].device
+        self.ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         base = (self.ws.data_ptr() + 255) // 256 * 256
         h = C.c_void_p()
-        check(lib.paci_pipeline_create(arr, S, base, nbytes, C.byref(h)), "paci_pipeline_create")
+        with torch.cuda.device(self.device):
+            check(lib.paci_pipeline_create(arr, S, base, nbytes, C.byref(h)), "paci_pipeline_create")
         self.handle = h
 
     def close(self):
@@ -245,8 +289,12 @@ class Pipeline:
 
     __del__ = close
 
-    def run(self, tokens, lr, mode=MODE_PACI, want_loss=True, want_delta=True):
-        """tokens: int32 [n, mu, T+1]; a torch CUDA tensor (resident) or a numpy / torch CPU array (host)."""
+    def run(self, tokens, lr, mode=MODE_PACI, want_loss=True, want_delta=True, n_seq=None, lr_by_update=None,
+            stream=None):
+        """tokens: int32 [n, mu, T+1]; a torch CUDA tensor (resident) or a numpy / torch CPU array (host).
+        n_seq: optional int32 [n] heterogeneous micro-batch sizes; lr_by_update: optional float32
+        array, the learning rate of each stage's u-th update during this run (PAPER.md:272 schedule).
+        The run is ordered after the work already enqueued on `stream` (default: torch's current stream)."""
         import torch
         S = len(self.stages)
         n = int(tokens.shape[0])
@@ -263,8 +311,17 @@ class Pipeline:
                         delta.ctypes.data_as(C.POINTER(C.c_int32)) if want_delta else None,
                         version.ctypes.data_as(C.POINTER(C.c_int64)), max_q.ctypes.data_as(C.POINTER(C.c_int32)),
                         0, 0, 0.0)
-        check(lib.paci_pipeline_run(self.handle, _ptr(tokens), int(on_host), n, mode, lr, C.byref(rep)),
-              "paci_pipeline_run")
+        sizes = None if n_seq is None else np.ascontiguousarray(n_seq, dtype=np.int32)
+        lrs = None if lr_by_update is None else np.ascontiguousarray(lr_by_update, dtype=np.float32)
+        with torch.cuda.device(self.device):
+            if sizes is None and lrs is None:
+                rc = lib.paci_pipeline_run(self.handle, _ptr(tokens), int(on_host), n, mode, lr, _stream(stream),
+                                           C.byref(rep))
+            else:
+                rc = lib.paci_pipeline_run_var(self.handle, _ptr(tokens), int(on_host), n, _ptr(sizes), mode, lr,
+                                               _ptr(lrs), 0 if lrs is None else lrs.size, _stream(stream),
+                                               C.byref(rep))
+        check(rc, "paci_pipeline_run")
         return dict(loss=loss, delta=delta, version=version, max_q=max_q, n_slots=rep.n_slots,
                     n_launches=rep.n_launches, elapsed_ms=rep.elapsed_ms)
 

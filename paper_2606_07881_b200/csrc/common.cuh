@@ -123,7 +123,9 @@ __device__ __forceinline__ float gelu_bf16(float p) {
 static inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }
 static inline size_t align_up(size_t a, size_t b) { return (a + b - 1) / b * b; }
 
-int num_sms();
+int num_sms();                                            // of the current device
+// cudaFuncAttributeMaxDynamicSharedMemorySize, once per (current device, kernel); thread-safe
+int set_max_dynamic_smem(const void* func, int bytes);
 
 // ---------------------------------------------------------------- sampled kernel timing (prof.cu)
 enum ProfCat { PC_GEMM_FWD = 0, PC_GEMM_DGRAD, PC_GEMM_WGRAD, PC_ATTN_FWD, PC_ATTN_BWD, PC_LN_FWD, PC_LN_BWD,
@@ -147,12 +149,18 @@ int gelu_fwd(int dtype, size_t n, const void* p, void* out, cudaStream_t s);
 int gelu_bwd(int dtype, int rows, int cols, const void* dg, const void* p, void* dp, float* Gbias,
              cudaStream_t s);
 int colsum(int dtype, int rows, int cols, const void* x, float* G, cudaStream_t s);
+// token / target ids outside [0, vocab) are clamped and raise *err (sticky device word, may be NULL)
 int embed_fwd(int dtype, int mu, int T, int D, const int32_t* tok, const float* wte, const float* wpe,
-              void* x, cudaStream_t s);
+              void* x, int vocab, int64_t* err, cudaStream_t s);
 int embed_bwd(int dtype, int mu, int T, int D, const int32_t* tok, const void* dx, float* Gwte,
-              float* Gwpe, cudaStream_t s);
-int softmax_ce(int dtype, int rows, int V, int ldz, void* z, const int32_t* tgt, float* loss,
+              float* Gwpe, int vocab, cudaStream_t s);
+int softmax_ce(int dtype, int rows, int V, int ldz, void* z, const int32_t* tgt, float* loss, int64_t* err,
                cudaStream_t s);
+// Dropout with a counter-based mask: element e of a [rows, cols] tensor is kept iff word (e % 4) of
+// Philox4x32-10(counter = (e / 4 lo, e / 4 hi, mb_id lo, site), key = seed) >= floor(p 2^32); kept values are
+// scaled by 1 / (1 - p).  out may alias x.  Forward and backward are the same map (the mask is regenerated).
+int dropout(int dtype, size_t n, const void* x, void* out, float p, uint64_t seed, int64_t mb_id, int site,
+            cudaStream_t s);
 int adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float* G, void* shadow, int k, int64_t t,
           float lr, float beta1, float beta2, float eps, float wd, int64_t* version_word, cudaStream_t s);
 int cast_shadow(size_t n, const float* w, void* shadow, cudaStream_t s);          // bf16 shadow of fp32
@@ -160,7 +168,7 @@ int stamp_version(const int64_t* version_word, int64_t* dst, cudaStream_t s);   
 int split_tokens(int mu, int T, const int32_t* tok_tp1, int32_t* inp, int32_t* tgt, cudaStream_t s);
 
 // GEMM: see paci_op_gemm in paci.h for layouts; lda/ldb/ldc are row strides in elements.
-// gemm() dispatches on dtype / backend.
+// gemm() dispatches on dtype.
 int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
          const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s);
 int gemm_simt(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
@@ -171,7 +179,7 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
 // one launch on the tcgen05 path (GELU in the GEMM epilogue, rows a7 + a8), GEMM then gelu_fwd otherwise.
 int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
                    void* C, void* Gout, int ldc, cudaStream_t s);
-bool gemm_backend_tcgen05();
+void gemm_tc_last_plan(int32_t* out6);
 int add_vec(int dtype, size_t n, const void* a, const void* b, void* out, cudaStream_t s);  // out = a (+ b)
 
 int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,

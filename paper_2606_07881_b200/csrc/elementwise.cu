@@ -4,7 +4,10 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdlib>
+#include <mutex>
+#include <set>
 #include <string>
+#include <utility>
 
 #include "common.cuh"
 #include "tc_ptx.cuh"
@@ -24,15 +27,34 @@ int fail(int code, const char* fmt, ...) {
   return code;
 }
 
+// Per-device state: the SM count and the "dynamic shared memory limit raised" flags are properties of a
+// (device, kernel) pair, so both are keyed by the CURRENT device, never cached process-wide.
+static constexpr int MAX_DEVICES = 64;
+
 int num_sms() {
-  static int n = 0;
-  if (n == 0) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-    if (n <= 0) n = 148;
+  static std::atomic<int> n[MAX_DEVICES];
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= MAX_DEVICES) dev = 0;
+  int v = n[dev].load(std::memory_order_relaxed);
+  if (v == 0) {
+    cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+    if (v <= 0) v = 148;
+    n[dev].store(v, std::memory_order_relaxed);
   }
-  return n;
+  return v;
+}
+
+int set_max_dynamic_smem(const void* func, int bytes) {
+  static std::mutex mu;
+  static std::set<std::pair<int, const void*>> done;
+  int dev = 0;
+  PACI_CUDA_OK(cudaGetDevice(&dev));
+  std::lock_guard<std::mutex> g(mu);
+  if (done.count({dev, func})) return PACI_OK;
+  PACI_CUDA_OK(cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+  done.insert({dev, func});
+  return PACI_OK;
 }
 
 __device__ __forceinline__ void red_add_v4(float* dst, float a, float b, float c, float d) {
@@ -232,16 +254,11 @@ static int ln_fwd_t(int rows, int D, const void* x, const void* res, const float
   constexpr int V = Vec<T>::N;
   if (D % V != 0) return fail(PACI_EINVAL, "layernorm: D=%d not a multiple of %d", D, V);
   if constexpr (sizeof(T) == 2) {
-    static const bool use_pipe = !(getenv("PACI_LN_FWD") && std::string(getenv("PACI_LN_FWD")) == "regs");
-    if (use_pipe && D == 1024 && rows % LNQ_R == 0 && (uintptr_t)x % 16 == 0 && (uintptr_t)res % 16 == 0) {
+    if (D == 1024 && rows % LNQ_R == 0 && (uintptr_t)x % 16 == 0 && (uintptr_t)res % 16 == 0) {
       constexpr int S = 12, SETS = 3;
       auto kern = ln_fwd_pipe_kernel<T, S, SETS>;
       const uint32_t smem = S * 2 * LNQ_R * (uint32_t)D * sizeof(T) + 2 * S * 8 + 64;
-      static bool attr_set = false;
-      if (!attr_set) {
-        PACI_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_set = true;
-      }
+      { int rc_ = set_max_dynamic_smem((const void*)kern, (int)smem); if (rc_) return rc_; }
       const int blocks = std::min(rows / LNQ_R, num_sms());
       PACI_LAUNCH(kern, blocks, (SETS * LNQ_R + 1) * 32, smem, s, rows, (const T*)x, (const T*)res, g, b, (T*)xsum, (T*)y,
                   mean, rstd);
@@ -701,10 +718,9 @@ static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float*
       (Gcol == nullptr || (uintptr_t)Gcol % 16 == 0)) {
     const int nw = D / (32 * V);
     // the shape the stage runs at (bf16, D = 1024): the bulk-copy pipelined kernel, one block per SM (8-stage ring of
-    // 4-row groups = 197 KB, 3 sets of 4 compute warps, 2 rows at a time); PACI_LN_BWD=regs keeps the kernel below
+    // 4-row groups = 197 KB, 3 sets of 4 compute warps, 2 rows at a time)
     if constexpr (sizeof(T) == 2) {
-      static const bool use_pipe = !(getenv("PACI_LN_BWD") && std::string(getenv("PACI_LN_BWD")) == "regs");
-      if (use_pipe && nw == 4 && rows % LNP_R == 0 && (uintptr_t)mean % 16 == 0 && (uintptr_t)rstd % 16 == 0 &&
+      if (nw == 4 && rows % LNP_R == 0 && (uintptr_t)mean % 16 == 0 && (uintptr_t)rstd % 16 == 0 &&
           (uintptr_t)dy % 16 == 0 && (uintptr_t)x % 16 == 0 && (uintptr_t)dres % 16 == 0) {
         // S is a multiple of SETS: every ring stage then belongs to ONE set, so each `full` barrier has a single
         // consumer sequence and a waiter can never be two phases behind it (parity waits cannot tell those apart)
@@ -713,11 +729,7 @@ static int ln_bwd_t(int rows, int D, const void* dy, const void* x, const float*
         auto kern = ln_bwd_pipe_kernel<T, 4, S, SETS, 2>;
         const uint32_t stage = 3 * LNP_R * (uint32_t)D * sizeof(T) + 32;
         const uint32_t smem = S * stage + 2 * S * 8 + 2 * SETS * LNP_R * 2 * 4 * 4 + 64;
-        static bool attr_set = false;
-        if (!attr_set) {
-          PACI_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-          attr_set = true;
-        }
+        { int rc_ = set_max_dynamic_smem((const void*)kern, (int)smem); if (rc_) return rc_; }
         const int blocks = std::min(rows / LNP_R, num_sms());
         PACI_LAUNCH(kern, blocks, (4 * SETS + 1) * 32, smem, s, rows, D, (const T*)dy, (const T*)x, mean, rstd, g,
                     (const T*)dres, (T*)dx, Gg, Gb, Gcol);
@@ -901,16 +913,24 @@ int colsum(int dtype, int rows, int cols, const void* x, float* G, cudaStream_t 
 }
 
 // =========================================================================== embedding
+// A token / target id outside [0, vocab) is clamped (no out-of-bounds access) and raises the stage's sticky
+// device error word, which paci_stage_check / paci_pipeline_run report as PACI_EINVAL.
+__device__ __forceinline__ int checked_id(int id, int vocab, int64_t* err) {
+  if ((unsigned)id < (unsigned)vocab) return id;
+  if (err != nullptr) *err = 1;
+  return id < 0 ? 0 : vocab - 1;
+}
 template <typename T>
 __global__ void __launch_bounds__(256) embed_fwd_kernel(int M, int T_, int D, const int32_t* __restrict__ tok,
                                                         const float* __restrict__ wte,
-                                                        const float* __restrict__ wpe, T* __restrict__ x) {
+                                                        const float* __restrict__ wpe, T* __restrict__ x,
+                                                        int vocab, int64_t* __restrict__ err) {
   constexpr int V = Vec<T>::N;
   const int nvec = D / V;
   const size_t total = (size_t)M * nvec;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
     const int row = (int)(i / nvec), c = (int)(i % nvec) * V;
-    const int id = tok[row], pos = row % T_;
+    const int id = checked_id(tok[row], vocab, err), pos = row % T_;
     float a[V], b[V];
     load_f32<V>(wte + (size_t)id * D + c, a);
     load_f32<V>(wpe + (size_t)pos * D + c, b);
@@ -921,22 +941,25 @@ __global__ void __launch_bounds__(256) embed_fwd_kernel(int M, int T_, int D, co
 }
 
 int embed_fwd(int dtype, int mu, int T_, int D, const int32_t* tok, const float* wte, const float* wpe, void* x,
-              cudaStream_t s) {
+              int vocab, int64_t* err, cudaStream_t s) {
   ProfScope prof(PC_EMBED, 0.0, ((dtype == PACI_BF16 ? 2.0 : 4.0) + 4.0) * mu * (double)T_ * D + 4.0 * T_ * D, s);
   const int M = mu * T_;
   const int V = dtype == PACI_BF16 ? 8 : 4;
   if (D % V) return fail(PACI_EINVAL, "embed: D=%d", D);
   const size_t total = (size_t)M * (D / V);
   int blocks = (int)std::min<size_t>((total + 255) / 256, (size_t)num_sms() * 16);
-  if (dtype == PACI_BF16) PACI_LAUNCH(embed_fwd_kernel<bf16>, blocks, 256, 0, s, M, T_, D, tok, wte, wpe, (bf16*)x);
-  else PACI_LAUNCH(embed_fwd_kernel<float>, blocks, 256, 0, s, M, T_, D, tok, wte, wpe, (float*)x);
+  if (dtype == PACI_BF16)
+    PACI_LAUNCH(embed_fwd_kernel<bf16>, blocks, 256, 0, s, M, T_, D, tok, wte, wpe, (bf16*)x, vocab, err);
+  else
+    PACI_LAUNCH(embed_fwd_kernel<float>, blocks, 256, 0, s, M, T_, D, tok, wte, wpe, (float*)x, vocab, err);
   return PACI_OK;
 }
 
 // Gwte[tok] += dx (fp32 vector atomics: red.global.add.v4.f32), Gwpe[t] += sum_b dx[b,t].
 template <typename T>
 __global__ void __launch_bounds__(256) embed_bwd_wte_kernel(int M, int D, const int32_t* __restrict__ tok,
-                                                            const T* __restrict__ dx, float* __restrict__ Gwte) {
+                                                            const T* __restrict__ dx, float* __restrict__ Gwte,
+                                                            int vocab) {
   constexpr int V = Vec<T>::N;
   const int nvec = D / V;
   const size_t total = (size_t)M * nvec;
@@ -944,7 +967,7 @@ __global__ void __launch_bounds__(256) embed_bwd_wte_kernel(int M, int D, const 
     const int row = (int)(i / nvec), c = (int)(i % nvec) * V;
     float v[V];
     load_vec<T>(dx + (size_t)row * D + c, v);
-    float* dst = Gwte + (size_t)tok[row] * D + c;
+    float* dst = Gwte + (size_t)checked_id(tok[row], vocab, nullptr) * D + c;
 #pragma unroll
     for (int j = 0; j < V; j += 4)
       asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(dst + j), "f"(v[j]), "f"(v[j + 1]),
@@ -976,7 +999,7 @@ __global__ void __launch_bounds__(256) embed_bwd_wpe_kernel(int mu, int T_, int 
 }
 
 int embed_bwd(int dtype, int mu, int T_, int D, const int32_t* tok, const void* dx, float* Gwte, float* Gwpe,
-              cudaStream_t s) {
+              int vocab, cudaStream_t s) {
   // dx read twice (wte scatter, wpe reduction) + fp32 read-modify-write of the touched rows
   ProfScope prof(PC_EMBED, 0.0, ((dtype == PACI_BF16 ? 2.0 : 4.0) * 2.0 + 8.0) * mu * (double)T_ * D + 8.0 * T_ * D, s);
   const int M = mu * T_;
@@ -986,10 +1009,10 @@ int embed_bwd(int dtype, int mu, int T_, int D, const int32_t* tok, const void* 
   int b1 = (int)std::min<size_t>((t1 + 255) / 256, (size_t)num_sms() * 16);
   int b2 = (int)std::min<size_t>((t2 + 255) / 256, (size_t)num_sms() * 16);
   if (dtype == PACI_BF16) {
-    PACI_LAUNCH(embed_bwd_wte_kernel<bf16>, b1, 256, 0, s, M, D, tok, (const bf16*)dx, Gwte);
+    PACI_LAUNCH(embed_bwd_wte_kernel<bf16>, b1, 256, 0, s, M, D, tok, (const bf16*)dx, Gwte, vocab);
     PACI_LAUNCH(embed_bwd_wpe_kernel<bf16>, b2, 256, 0, s, mu, T_, D, (const bf16*)dx, Gwpe);
   } else {
-    PACI_LAUNCH(embed_bwd_wte_kernel<float>, b1, 256, 0, s, M, D, tok, (const float*)dx, Gwte);
+    PACI_LAUNCH(embed_bwd_wte_kernel<float>, b1, 256, 0, s, M, D, tok, (const float*)dx, Gwte, vocab);
     PACI_LAUNCH(embed_bwd_wpe_kernel<float>, b2, 256, 0, s, mu, T_, D, (const float*)dx, Gwpe);
   }
   return PACI_OK;
@@ -1006,7 +1029,7 @@ template <> __device__ __forceinline__ float exp_t<bf16>(float x) { return __exp
 template <typename T>
 __global__ void __launch_bounds__(512) softmax_ce_kernel(int rows, int V_, int ldz, T* __restrict__ z,
                                                          const int32_t* __restrict__ tgt,
-                                                         float* __restrict__ loss) {
+                                                         float* __restrict__ loss, int64_t* __restrict__ err) {
   constexpr int V = Vec<T>::N;
   __shared__ float red_m[16], red_s[16];
   __shared__ float sh_max, sh_sum;
@@ -1045,7 +1068,7 @@ __global__ void __launch_bounds__(512) softmax_ce_kernel(int rows, int V_, int l
   }
   __syncthreads();
   const float bm = sh_max, inv = 1.f / sh_sum, scale = 1.f / (float)rows;
-  const int t = tgt[row];
+  const int t = checked_id(tgt[row], V_, threadIdx.x == 0 ? err : nullptr);
   if (threadIdx.x == 0) {
     const float zt = to_f(zr[t]);
     atomicAdd(loss, (logf(sh_sum) + bm - zt) * scale);
@@ -1065,12 +1088,13 @@ __global__ void __launch_bounds__(512) softmax_ce_kernel(int rows, int V_, int l
   }
 }
 
-int softmax_ce(int dtype, int rows, int V_, int ldz, void* z, const int32_t* tgt, float* loss, cudaStream_t s) {
+int softmax_ce(int dtype, int rows, int V_, int ldz, void* z, const int32_t* tgt, float* loss, int64_t* err,
+               cudaStream_t s) {
   ProfScope prof(PC_SOFTMAX_CE, 0.0, (dtype == PACI_BF16 ? 2.0 : 4.0) * 2.0 * rows * (double)ldz, s);
   const int V = dtype == PACI_BF16 ? 8 : 4;
   if (ldz % V || ldz < V_) return fail(PACI_EINVAL, "softmax_ce: ldz=%d V=%d", ldz, V_);
-  if (dtype == PACI_BF16) PACI_LAUNCH(softmax_ce_kernel<bf16>, rows, 512, 0, s, rows, V_, ldz, (bf16*)z, tgt, loss);
-  else PACI_LAUNCH(softmax_ce_kernel<float>, rows, 512, 0, s, rows, V_, ldz, (float*)z, tgt, loss);
+  if (dtype == PACI_BF16) PACI_LAUNCH(softmax_ce_kernel<bf16>, rows, 512, 0, s, rows, V_, ldz, (bf16*)z, tgt, loss, err);
+  else PACI_LAUNCH(softmax_ce_kernel<float>, rows, 512, 0, s, rows, V_, ldz, (float*)z, tgt, loss, err);
   return PACI_OK;
 }
 
@@ -1135,6 +1159,62 @@ int cast_shadow(size_t n, const float* w, void* shadow, cudaStream_t s) {
   ProfScope prof(PC_OTHER, 0.0, 6.0 * (double)n, s);
   int blocks = (int)std::min<size_t>((n + 255) / 256, (size_t)num_sms() * 8);
   PACI_LAUNCH(cast_shadow_kernel, blocks, 256, 0, s, n, w, (bf16*)shadow);
+  return PACI_OK;
+}
+
+// =========================================================================== dropout
+// Philox4x32-10 (Salmon et al., "Parallel random numbers: as easy as 1, 2, 3"): 10 rounds of
+//   (c0, c1, c2, c3) <- (hi(M1 c2) ^ c1 ^ k0, lo(M1 c2), hi(M0 c0) ^ c3 ^ k1, lo(M0 c0)),  k += (W0, W1) between rounds.
+// The oracle evaluates the same generator on the same counters (oracle/dropout.py), so the masks agree bit for bit.
+struct Philox4 { uint32_t v[4]; };
+__device__ __forceinline__ Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                                 uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    c0 = hi1 ^ c1 ^ k0; c1 = lo1; c2 = hi0 ^ c3 ^ k1; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  return Philox4{{c0, c1, c2, c3}};
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256) dropout_kernel(size_t nvec, const T* __restrict__ x, T* __restrict__ out,
+                                                      uint32_t thresh, float scale, uint32_t k0, uint32_t k1,
+                                                      uint32_t mb, uint32_t site) {
+  constexpr int V = Vec<T>::N;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+    float v[V];
+    load_vec<T>(x + i * V, v);
+#pragma unroll
+    for (int q = 0; q < V / 4; ++q) {
+      const uint64_t blk = i * (V / 4) + q;                  // element index / 4
+      const Philox4 r = philox4x32_10((uint32_t)blk, (uint32_t)(blk >> 32), mb, site, k0, k1);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) v[4 * q + j] = r.v[j] >= thresh ? v[4 * q + j] * scale : 0.f;
+    }
+    store_vec<T>(out + i * V, v);
+  }
+}
+
+int dropout(int dtype, size_t n, const void* x, void* out, float p, uint64_t seed, int64_t mb_id, int site,
+            cudaStream_t s) {
+  if (n == 0) return PACI_OK;
+  if (!(p >= 0.f && p < 1.f)) return fail(PACI_EINVAL, "dropout: p=%f", (double)p);
+  ProfScope prof(PC_OTHER, 0.0, (dtype == PACI_BF16 ? 2.0 : 4.0) * 2.0 * (double)n, s);
+  const int V = dtype == PACI_BF16 ? 8 : 4;
+  if (n % V) return fail(PACI_EINVAL, "dropout: n not a multiple of %d", V);
+  const size_t nvec = n / V;
+  const uint32_t thresh = (uint32_t)std::min<double>(std::floor((double)p * 4294967296.0), 4294967295.0);
+  const float scale = 1.f / (1.f - p);
+  int blocks = (int)std::min<size_t>((nvec + 255) / 256, (size_t)num_sms() * 16);
+  if (dtype == PACI_BF16)
+    PACI_LAUNCH(dropout_kernel<bf16>, blocks, 256, 0, s, nvec, (const bf16*)x, (bf16*)out, thresh, scale,
+                (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)mb_id, (uint32_t)site);
+  else
+    PACI_LAUNCH(dropout_kernel<float>, blocks, 256, 0, s, nvec, (const float*)x, (float*)out, thresh, scale,
+                (uint32_t)seed, (uint32_t)(seed >> 32), (uint32_t)mb_id, (uint32_t)site);
   return PACI_OK;
 }
 

@@ -409,11 +409,7 @@ int launch(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tm
                           EPI_STAGING_BYTES + 4 * BLOCK_N * 4 + 1024 + 256;
   static_assert(SMEM <= 232448, "shared memory budget of one sm_100 CTA");
   auto kern = gemm_tc_kernel<CG, BLOCK_N, STAGES, A_MN, B_MN, ACCUM>;
-  static bool attr_set = false;
-  if (!attr_set) {
-    PACI_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM));
-    attr_set = true;
-  }
+  { int rc_ = set_max_dynamic_smem((const void*)kern, (int)SMEM); if (rc_) return rc_; }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(grid);
   cfg.blockDim = dim3(NUM_THREADS);
@@ -431,14 +427,7 @@ int launch(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tm
   return PACI_OK;
 }
 
-// PACI_GEMM_CG=1 selects the single-CTA kernel (A/B comparison aid); default is the CTA-pair kernel.
-int cta_group() {
-  static const int cg = [] {
-    const char* e = std::getenv("PACI_GEMM_CG");
-    return (e != nullptr && e[0] == '1') ? 1 : 2;
-  }();
-  return cg;
-}
+thread_local int32_t g_last_plan[6] = {0, 0, 0, 0, 0, 0};
 
 }  // namespace
 
@@ -458,7 +447,7 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
     return fail(PACI_EINVAL, "tcgen05 GEMM: C not 16-byte aligned (ldc=%d)", ldc);
   if (bias != nullptr && (uintptr_t)bias % 16) return fail(PACI_EINVAL, "tcgen05 GEMM: bias not 16-byte aligned");
   const bool a_mn = layout == 2, b_mn = layout != 0;
-  const int CG = cta_group();
+  constexpr int CG = 2;                              // CTA pair (cluster of 2, one TPC) per 256-row tile
   const int BN = N <= 128 ? 128 : 256;
   CUtensorMap tmA, tmB, tmC, tmC2;
   int rc;
@@ -497,7 +486,7 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
   }
   p.splits = splits;
   p.range_mode = 0;
-  if (out_f32_accum && getenv("PACI_GEMM_RANGE") == nullptr) {
+  if (out_f32_accum) {
     // equal contiguous (tile, k-block) ranges instead of whole items: U / W k-blocks per worker plus one flush per
     // tile boundary crossed (+1).  Taken for outputs of many rounds (the LM-head wgrad: 788 tiles, 10.65 rounds ->
     // 0.659 to 0.597 ms); with fewer tiles than two rounds the k-block rate itself drops when every pair is busy
@@ -526,14 +515,16 @@ int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void*
     if (layout == 1) GO(CG_, BN_, ST_, false, true, false);                                               \
     GO(CG_, BN_, ST_, true, true, false);                                                                 \
   } while (0)
-  if (CG == 2) {
-    if (BN == 128) BY_LAYOUT(2, 128, 7);
-    BY_LAYOUT(2, 256, 5);
-  }
-  if (BN == 128) BY_LAYOUT(1, 128, 5);
-  BY_LAYOUT(1, 256, 3);
+  g_last_plan[0] = CG; g_last_plan[1] = BN; g_last_plan[2] = splits; g_last_plan[3] = p.range_mode;
+  g_last_plan[4] = grid; g_last_plan[5] = tiles;
+  if (BN == 128) BY_LAYOUT(2, 128, 7);
+  BY_LAYOUT(2, 256, 5);
 #undef BY_LAYOUT
 #undef GO
+}
+
+void gemm_tc_last_plan(int32_t* out6) {
+  for (int i = 0; i < 6; ++i) out6[i] = g_last_plan[i];
 }
 
 }  // namespace paci

@@ -1,4 +1,5 @@
-// ops.cu -- backend dispatch (fp32 -> FFMA kernels, bf16 -> tcgen05 / tensor-core kernels) and the
+// ops.cu -- dispatch on the stage's dtype (PACI_FP32 -> the FFMA parity kernels, PACI_BF16 -> the tcgen05 kernels;
+// one kernel family per dtype, no switches) and the
 // op-level C-ABI entry points used by the kernel parity tests and the per-kernel roofline benches.
 #include <algorithm>
 #include <cstdlib>
@@ -8,40 +9,19 @@
 
 namespace paci {
 
-static bool env_is(const char* name, const char* val) {
-  const char* e = std::getenv(name);
-  return e != nullptr && std::strcmp(e, val) == 0;
-}
-
-// PACI_GEMM=simt / PACI_ATTN=simt force the CUDA-core kernels in bf16 mode: a debugging aid to
-// bisect a parity failure, reported by paci_gemm_backend_is_tcgen05(); never selected silently.
-bool gemm_backend_tcgen05() {
-  static const bool simt = env_is("PACI_GEMM", "simt");
-  return !simt;
-}
-static bool attn_backend_tensor() {
-  static const bool simt = env_is("PACI_ATTN", "simt");
-  return !simt;
-}
-// PACI_ATTN=mma keeps the warp-level mma.sync kernels even where the tcgen05 kernels apply (T % 128 == 0)
-static bool attn_backend_tcgen05() {
-  static const bool off = env_is("PACI_ATTN", "mma") || env_is("PACI_ATTN", "simt");
-  return !off;
-}
-
 int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
          const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s) {
   const double e = dtype == PACI_BF16 ? 2.0 : 4.0;
   ProfScope prof(layout == 0 ? PC_GEMM_FWD : layout == 1 ? PC_GEMM_DGRAD : PC_GEMM_WGRAD, 2.0 * M * N * K,
                  e * ((double)M * K + (double)N * K) + (out_f32_accum ? 8.0 : e) * M * N, s);
-  if (dtype == PACI_BF16 && gemm_backend_tcgen05())
+  if (dtype == PACI_BF16)
     return gemm_tc(layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, s);
   return gemm_simt(dtype, layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, s);
 }
 
 int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
                    void* C, void* Gout, int ldc, cudaStream_t s) {
-  if (dtype == PACI_BF16 && gemm_backend_tcgen05()) {
+  if (dtype == PACI_BF16) {
     ProfScope prof(PC_GEMM_FWD, 2.0 * M * N * K, 2.0 * ((double)M * K + (double)N * K) + 4.0 * M * N, s);
     return gemm_tc(0, M, N, K, A, lda, B, ldb, bias, C, ldc, 0, s, Gout);
   }
@@ -51,52 +31,43 @@ int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const
   return gelu_fwd(dtype, (size_t)M * N, C, Gout, s);
 }
 
-int attention_fwd_mma(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
 int attention_fwd_tc(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
 int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
                      void* dqkv, float* scratch, float* Gbias, cudaStream_t s);
-int attention_bwd_mma(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
-                      void* dqkv, float* scratch, cudaStream_t s);
-size_t attention_bwd_mma_scratch_bytes(int mu, int T, int H);
 size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H);
 
 // algorithmic work: causal half of QK^T and PV (2 * mu*H*T*T*dh flops forward, twice that backward)
 int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse, cudaStream_t s) {
   const double e = dtype == PACI_BF16 ? 2.0 : 4.0, nd = (double)mu * T * H * dh;
   ProfScope prof(PC_ATTN_FWD, 2.0 * mu * H * (double)T * T * dh, e * 4.0 * nd + 4.0 * mu * H * T, s);
-  if (dtype == PACI_BF16 && attn_backend_tensor()) {
-    if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
-    if (T % 128 == 0 && attn_backend_tcgen05()) return attention_fwd_tc(mu, T, H, qkv, o, lse, s);
-    return attention_fwd_mma(mu, T, H, qkv, o, lse, s);
+  if (dtype == PACI_BF16) {
+    if (dh != 64 || T % 128) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 128 == 0");
+    return attention_fwd_tc(mu, T, H, qkv, o, lse, s);
   }
   return attention_fwd_simt(dtype, mu, T, H, dh, qkv, o, lse, s);
 }
 
 // Gbias (fp32 [3 H dh], may be NULL) += column sums of dqkv: the QKV bias gradient (row a15).  The tcgen05
-// kernels take it in their epilogue; the other backends run the column-sum kernel over dqkv afterwards.
+// kernels take it in their epilogue; the fp32 parity kernels run the column-sum kernel over dqkv afterwards.
 int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv, const void* o,
                   const float* lse, void* dqkv, float* scratch, float* Gbias, cudaStream_t s) {
   int rc;
   {
     const double e = dtype == PACI_BF16 ? 2.0 : 4.0, nd = (double)mu * T * H * dh;
     ProfScope prof(PC_ATTN_BWD, 4.0 * mu * H * (double)T * T * dh, e * 8.0 * nd + 4.0 * mu * H * T, s);
-    if (dtype == PACI_BF16 && attn_backend_tensor()) {
-      if (dh != 64 || T % 64) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 64 == 0");
-      if (T % 128 == 0 && attn_backend_tcgen05())
-        return attention_bwd_tc(mu, T, H, dout, qkv, o, lse, dqkv, scratch, Gbias, s);
-      rc = attention_bwd_mma(mu, T, H, dout, qkv, o, lse, dqkv, scratch, s);
-    } else {
-      rc = attention_bwd_simt(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, s);
+    if (dtype == PACI_BF16) {
+      if (dh != 64 || T % 128) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 128 == 0");
+      return attention_bwd_tc(mu, T, H, dout, qkv, o, lse, dqkv, scratch, Gbias, s);
     }
+    rc = attention_bwd_simt(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, s);
   }
   if (rc == PACI_OK && Gbias != nullptr) rc = colsum(dtype, mu * T, 3 * H * dh, dqkv, Gbias, s);
   return rc;
 }
 
 size_t attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh) {
-  size_t simt = (size_t)mu * H * T * sizeof(float);
-  if (dtype == PACI_BF16 && dh == 64)
-    return std::max({simt, attention_bwd_mma_scratch_bytes(mu, T, H), attention_bwd_tc_scratch_bytes(mu, T, H)});
+  const size_t simt = (size_t)mu * H * T * sizeof(float);
+  if (dtype == PACI_BF16 && dh == 64) return std::max(simt, attention_bwd_tc_scratch_bytes(mu, T, H));
   return simt;
 }
 
@@ -144,17 +115,21 @@ int paci_op_attention_bwd(int dtype, int mu, int T, int H, int dh, const void* d
 size_t paci_op_attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh) {
   return attention_bwd_scratch_bytes(dtype, mu, T, H, dh);
 }
-int paci_op_embed_fwd(int dtype, int mu, int T, int D, const int32_t* tok, const float* wte, const float* wpe,
-                      void* x, void* stream) {
-  return embed_fwd(dtype, mu, T, D, tok, wte, wpe, x, (cudaStream_t)stream);
+int paci_op_embed_fwd(int dtype, int mu, int T, int D, int vocab, const int32_t* tok, const float* wte,
+                      const float* wpe, void* x, void* stream) {
+  return embed_fwd(dtype, mu, T, D, tok, wte, wpe, x, vocab, nullptr, (cudaStream_t)stream);
 }
-int paci_op_embed_bwd(int dtype, int mu, int T, int D, const int32_t* tok, const void* dx, float* Gwte,
+int paci_op_embed_bwd(int dtype, int mu, int T, int D, int vocab, const int32_t* tok, const void* dx, float* Gwte,
                       float* Gwpe, void* stream) {
-  return embed_bwd(dtype, mu, T, D, tok, dx, Gwte, Gwpe, (cudaStream_t)stream);
+  return embed_bwd(dtype, mu, T, D, tok, dx, Gwte, Gwpe, vocab, (cudaStream_t)stream);
 }
 int paci_op_softmax_ce(int dtype, int rows, int V, int ldz, void* z, const int32_t* tgt, float* loss,
                        void* stream) {
-  return softmax_ce(dtype, rows, V, ldz, z, tgt, loss, (cudaStream_t)stream);
+  return softmax_ce(dtype, rows, V, ldz, z, tgt, loss, nullptr, (cudaStream_t)stream);
+}
+int paci_op_dropout(int dtype, size_t n, const void* x, void* out, float p, uint64_t seed, int64_t mb_id,
+                    int32_t site, void* stream) {
+  return dropout(dtype, n, x, out, p, seed, mb_id, site, (cudaStream_t)stream);
 }
 int paci_op_adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float* G, void* shadow_bf16, int k,
                   int64_t t, float lr, float beta1, float beta2, float eps, float weight_decay,

@@ -33,7 +33,7 @@ struct paci_pipeline {
   int tok_ring;
   int32_t *tok_stage, *tok_in, *tok_tgt;               // [tok_ring][mu*(T+1)], [tok_ring][M], [tok_ring][M]
   float* loss;                                         // [MAX_MB]
-  cudaEvent_t ev_start, ev_stop;
+  cudaEvent_t ev_start, ev_stop, ev_in;
   std::vector<cudaEvent_t> ev_done;
 };
 
@@ -119,6 +119,7 @@ int paci_pipeline_create(paci_stage_t* const* stages, int32_t n_stages, void* de
     return rc;
   PACI_CUDA_OK(cudaEventCreate(&p->ev_start));
   PACI_CUDA_OK(cudaEventCreate(&p->ev_stop));
+  PACI_CUDA_OK(cudaEventCreateWithFlags(&p->ev_in, cudaEventDisableTiming));
   *out = p;
   return PACI_OK;
 }
@@ -131,15 +132,26 @@ int paci_pipeline_destroy(paci_pipeline_t* p) {
     for (auto e : *v) cudaEventDestroy(e);
   cudaEventDestroy(p->ev_start);
   cudaEventDestroy(p->ev_stop);
+  cudaEventDestroy(p->ev_in);
   delete p;
   return PACI_OK;
 }
 
 int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_on_host, int64_t n,
-                      int32_t mode, float lr, paci_run_report* rep) {
+                      int32_t mode, float lr, void* stream, paci_run_report* rep) {
+  return paci_pipeline_run_var(p, tokens, tokens_on_host, n, nullptr, mode, lr, nullptr, 0, stream, rep);
+}
+
+int paci_pipeline_run_var(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_on_host, int64_t n,
+                          const int32_t* n_seq, int32_t mode, float lr, const float* lr_by_update,
+                          int64_t n_updates, void* stream, paci_run_report* rep) {
   if (!p || !tokens || !rep) return fail(PACI_EINVAL, "null pointer");
   if (n < 0 || n > MAX_MB) return fail(PACI_EINVAL, "n_microbatches %lld out of range", (long long)n);
   if (mode != PACI_MODE_PACI && mode != PACI_MODE_FLUSH) return fail(PACI_EINVAL, "mode %d", mode);
+  if (n_seq)
+    for (int64_t m = 0; m < n; ++m)
+      if (n_seq[m] < 1 || n_seq[m] > p->mu)
+        return fail(PACI_EINVAL, "n_seq[%lld] = %d outside [1, %d]", (long long)m, n_seq[m], p->mu);
   const int S = p->S, M = p->mu * p->T;
   const size_t tok_per_mb = (size_t)p->mu * (p->T + 1);
   for (int s = 0; s < S; ++s)
@@ -153,7 +165,10 @@ int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_
     explicit PeerGuard(const std::vector<cudaStream_t>& v) { prof_set_peer_streams(v.data(), (int)v.size()); }
     ~PeerGuard() { prof_set_peer_streams(nullptr, 0); }
   } peer_guard(p->streams);
-  // all stage streams start after ev_start
+  // the run is ordered after everything already enqueued on the caller's stream (e.g. the producer of a device
+  // token buffer); all stage streams start after ev_start
+  PACI_CUDA_OK(cudaEventRecord(p->ev_in, (cudaStream_t)stream));
+  PACI_CUDA_OK(cudaStreamWaitEvent(p->main, p->ev_in, 0));
   PACI_CUDA_OK(cudaEventRecord(p->ev_start, p->main));
   for (int s = 0; s < S; ++s) PACI_CUDA_OK(cudaStreamWaitEvent(p->streams[s], p->ev_start, 0));
 
@@ -191,7 +206,14 @@ int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_
         if (s < S - 1) PACI_CUDA_OK(cudaEventRecord(p->b_free[s * RING + r], cs));
         if (s > 0) PACI_CUDA_OK(cudaEventRecord(p->b_ready[(s - 1) * RING + r], cs));
         if (rep->delta) rep->delta[(size_t)s * n + m] = paci_crossed_updates(p->st[s], m);
-        rc = paci_maybe_step(p->st[s], lr, cs);
+        float lr_now = lr;                                   // LR schedule: indexed by the stage's own update count
+        if (lr_by_update) {
+          const int64_t u = paci_version(p->st[s]) - v0[s];
+          if (paci_window_count(p->st[s]) == p->k && u >= n_updates)
+            return fail(PACI_EINVAL, "pipeline_run: lr_by_update has %lld entries, update %lld needed", (long long)n_updates, (long long)u);
+          if (u < n_updates) lr_now = lr_by_update[u];
+        }
+        rc = paci_maybe_step(p->st[s], lr_now, cs);
         if (rc < 0) return rc;
         nb[s] += 1;
         if (s > 0) new_b[s - 1] += 1;
@@ -213,7 +235,7 @@ int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_
             PACI_CUDA_OK(cudaMemcpyAsync(stg, src, tok_per_mb * 4, cudaMemcpyHostToDevice, cs));
             src = stg;
           }
-          int rc = split_tokens(p->mu, p->T, src, p->tok_in + (size_t)tr * M, p->tok_tgt + (size_t)tr * M, cs);
+          int rc = split_tokens(n_seq ? n_seq[m] : p->mu, p->T, src, p->tok_in + (size_t)tr * M, p->tok_tgt + (size_t)tr * M, cs);
           if (rc != PACI_OK) return rc;
           in = p->tok_in + (size_t)tr * M;
         } else {
@@ -227,7 +249,7 @@ int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_
           if (m >= RING) PACI_CUDA_OK(cudaStreamWaitEvent(cs, p->f_free[s * RING + r], 0));
           outp = p->fbuf[s * RING + r];
         }
-        int rc = paci_forward(p->st[s], m, in, tgt, outp, cs);
+        int rc = paci_forward_var(p->st[s], m, n_seq ? n_seq[m] : p->mu, in, tgt, outp, cs);
         if (rc != PACI_OK) return rc;   // EAGAIN cannot happen after the probe above
         if (s > 0) PACI_CUDA_OK(cudaEventRecord(p->f_free[(s - 1) * RING + r], cs));
         if (s < S - 1) PACI_CUDA_OK(cudaEventRecord(p->f_ready[s * RING + r], cs));
@@ -253,6 +275,10 @@ int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_
     PACI_CUDA_OK(cudaMemcpyAsync(rep->loss, p->loss, (size_t)n * 4, cudaMemcpyDeviceToHost, p->main));
   PACI_CUDA_OK(cudaStreamSynchronize(p->main));
   PACI_CUDA_OK(cudaEventElapsedTime(&rep->elapsed_ms, p->ev_start, p->ev_stop));
+  for (int s : {0, S - 1}) {                               // device-side validation of token / target ids
+    int rc = paci_stage_check(p->st[s], p->main);
+    if (rc != PACI_OK) return rc;
+  }
   rep->n_slots = slots;
   rep->n_launches = paci_launch_count() - launches0;
   for (int s = 0; s < S; ++s) {

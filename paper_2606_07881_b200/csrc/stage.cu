@@ -10,6 +10,7 @@
 //   ctl            device version word, (vF, vB) stamps
 //   stash          S-s slots ("the first stage carries N microbatches, the last carries one")
 //   scratch        forward / backward temporaries
+#include <cmath>
 #include <cstring>
 #include <deque>
 #include <unordered_map>
@@ -35,32 +36,45 @@ static constexpr int LOG_CAP = 4096;
 
 using namespace paci;
 
+namespace paci {
+struct Wref {   // pointers to one tensor in every group
+  float* w; float* g; const void* wc;   // master, grad accumulator, compute-dtype weights (shadow or master)
+};
+struct BlockW { Wref ln1g, ln1b, wqkv, bqkv, wo, bo, ln2g, ln2b, w1, b1, w2, b2; };
+}  // namespace paci
+
 struct paci_stage {
   paci_stage_config cfg;
   int dtype, L, D, H, dh, T, mu, M, V, Vpad, S, s, k;
   size_t esz;
   std::vector<TensorInfo> tensors;
   std::unordered_map<std::string, int> index;
+  std::vector<BlockW> bw;                          // per-block pointer table, built once at create
+  Wref wte, wpe, lnfg, lnfb, head;
   size_t P, n_decay;
   // device
   char* ws;
   float *W, *Mo, *Vo, *G;
   bf16* Wb;
   int64_t* dev_version;
+  int64_t* dev_err;        // sticky: a token / target id was out of range
   int64_t* dev_stamps;     // [LOG_CAP][2]
   int n_slots;
-  size_t slot_bytes;
+  size_t slot_bytes;       // of a stash slot: the full activation set, or (checkpoint) the stage input only
   char* stash;
+  char* work_slot;         // checkpoint mode: the ONE full activation set, shared by forward and recompute
+  size_t ck_in, ck_tgt;    // checkpoint mode: offsets of the stage input / targets inside a stash slot
   std::vector<BlockStash> bs;
   size_t off_tok, off_xf_in, off_xf, off_meanf, off_rstdf, off_z;
   // scratch
-  char *sc_proj, *sc_emb, *sc_dxa, *sc_dxb, *sc_dx1, *sc_dD, *sc_dD2, *sc_d4, *sc_dqkv;
+  char *sc_proj, *sc_emb, *sc_dxa, *sc_dxb, *sc_dx1, *sc_dD, *sc_dD2, *sc_d4, *sc_dqkv, *sc_dmask;
   float* sc_attn;
+  float* sc_loss;
   // host state (Alg. 1 lines 1-3 + P:66)
   int64_t version;
   int q, c;
   int64_t n_forwards;
-  struct Unresolved { int64_t mb; int slot; int64_t vF; int log_idx; };
+  struct Unresolved { int64_t mb; int slot; int64_t vF; int log_idx; int n_seq; };
   std::deque<Unresolved> fifo;
   struct LogEntry { int64_t mb; int32_t delta; bool done; };
   std::vector<LogEntry> log;                       // ring, index = forward ordinal % LOG_CAP
@@ -116,7 +130,7 @@ static int validate(const paci_stage_config* c) {
   if (c->dtype == PACI_BF16) {
     if (c->d_model % 64) return fail(PACI_EINVAL, "PACI_BF16 needs d_model %% 64 == 0");
     if (dh != 64) return fail(PACI_EINVAL, "PACI_BF16 needs head dim 64 (got %d)", dh);
-    if (c->seq_len % 64) return fail(PACI_EINVAL, "PACI_BF16 needs seq_len %% 64 == 0");
+    if (c->seq_len % 128) return fail(PACI_EINVAL, "PACI_BF16 needs seq_len %% 128 == 0");
   } else if (c->dtype == PACI_FP32) {
     if (c->d_model % 4 || dh > 128) return fail(PACI_EINVAL, "PACI_FP32 needs d_model %% 4 == 0, head dim <= 128");
   } else {
@@ -124,15 +138,19 @@ static int validate(const paci_stage_config* c) {
   }
   if ((c->has_embedding || c->has_head) && c->vocab <= 0) return fail(PACI_EINVAL, "vocab");
   if (c->n_layers == 0 && !c->has_embedding && !c->has_head) return fail(PACI_EINVAL, "empty stage");
+  if (c->checkpoint != 0 && c->checkpoint != 1) return fail(PACI_EINVAL, "checkpoint %d", c->checkpoint);
+  if (!(c->dropout_p >= 0.f && c->dropout_p < 1.f)) return fail(PACI_EINVAL, "dropout_p %f", (double)c->dropout_p);
   return PACI_OK;
 }
 
 struct Layout {
-  size_t P, n_decay, off_W, off_M, off_V, off_G, off_Wb, off_ctl, off_stash, slot_bytes, off_scratch, total;
+  size_t P, n_decay, off_W, off_M, off_V, off_G, off_Wb, off_ctl, off_stash, slot_bytes, full_slot_bytes, off_scratch,
+      total;
   int n_slots, Vpad;
   std::vector<BlockStash> bs;
   size_t off_tok, off_xf_in, off_xf, off_meanf, off_rstdf, off_z;
-  size_t sc_proj, sc_emb, sc_dxa, sc_dxb, sc_dx1, sc_dD, sc_dD2, sc_d4, sc_dqkv, sc_attn;
+  size_t ck_in, ck_tgt, work_slot;
+  size_t sc_proj, sc_emb, sc_dxa, sc_dxb, sc_dx1, sc_dD, sc_dD2, sc_d4, sc_dqkv, sc_attn, sc_dmask, sc_loss;
 };
 
 static Layout make_layout(const paci_stage_config& c) {
@@ -145,8 +163,8 @@ static Layout make_layout(const paci_stage_config& c) {
   auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
   L.off_W = take(L.P * 4); L.off_M = take(L.P * 4); L.off_V = take(L.P * 4); L.off_G = take(L.P * 4);
   L.off_Wb = take(c.dtype == PACI_BF16 ? L.P * 2 : 0);
-  L.off_ctl = take(8 + (size_t)LOG_CAP * 2 * 8);
-  // one stash slot
+  L.off_ctl = take(16 + (size_t)LOG_CAP * 2 * 8);
+  // one full activation set ("activations required for backpropagation", Alg. 1 line 7)
   size_t so = 0;
   auto stake = [&](size_t bytes) { size_t o = so; so = align_up(so + bytes, 256); return o; };
   L.off_tok = stake(c.has_embedding ? M * 4 : 0);
@@ -163,15 +181,24 @@ static Layout make_layout(const paci_stage_config& c) {
   L.off_meanf = stake(c.has_head ? M * 4 : 0);
   L.off_rstdf = stake(c.has_head ? M * 4 : 0);
   L.off_z = stake(c.has_head ? M * (size_t)L.Vpad * e : 0);
-  L.slot_bytes = so;
+  L.full_slot_bytes = so;
+  // checkpoint mode: a stash slot holds the stage input (and the targets) only
+  size_t co = 0;
+  auto ctake = [&](size_t bytes) { size_t o = co; co = align_up(co + bytes, 256); return o; };
+  L.ck_in = ctake(c.has_embedding ? M * 4 : M * D * e);
+  L.ck_tgt = ctake(c.has_head ? M * 4 : 0);
+  L.slot_bytes = c.checkpoint ? co : so;
   L.n_slots = c.n_stages - c.stage_index;          // d_s + 1 (Eq. 9: q <= d_s before admission)
   L.off_stash = take(L.slot_bytes * L.n_slots);
+  L.work_slot = take(c.checkpoint ? L.full_slot_bytes : 0);
   L.off_scratch = off;
   L.sc_proj = take(M * D * e); L.sc_emb = take(c.has_embedding ? M * D * e : 0);
   L.sc_dxa = take(M * D * e); L.sc_dxb = take(M * D * e); L.sc_dx1 = take(M * D * e);
   L.sc_dD = take(M * D * e);  L.sc_dD2 = take(M * D * e); L.sc_d4 = take(M * 4 * D * e);
   L.sc_dqkv = take(M * 3 * D * e);
   L.sc_attn = take(attention_bwd_scratch_bytes(c.dtype, c.micro_batch, c.seq_len, c.n_heads, D / c.n_heads));
+  L.sc_dmask = take(c.dropout_p > 0.f ? M * D * e : 0);
+  L.sc_loss = take(256);
   L.total = off;
   return L;
 }
@@ -182,7 +209,7 @@ extern "C" {
 
 const char* paci_last_error(void) { return g_last_error.c_str(); }
 int64_t paci_launch_count(void) { return g_launches.load(); }
-int paci_gemm_backend_is_tcgen05(void) { return gemm_backend_tcgen05() ? 1 : 0; }
+void paci_gemm_last_plan(int32_t* out6) { if (out6) gemm_tc_last_plan(out6); }
 
 size_t paci_stage_workspace_bytes(const paci_stage_config* cfg) {
   if (validate(cfg) != PACI_OK) return 0;
@@ -216,8 +243,13 @@ int paci_stage_create(const paci_stage_config* cfg, void* dev_ws, size_t ws_byte
   st->G = (float*)(st->ws + L.off_G);
   st->Wb = cfg->dtype == PACI_BF16 ? (bf16*)(st->ws + L.off_Wb) : nullptr;
   st->dev_version = (int64_t*)(st->ws + L.off_ctl);
-  st->dev_stamps = st->dev_version + 1;
+  st->dev_err = st->dev_version + 1;
+  st->dev_stamps = st->dev_version + 2;
   st->n_slots = L.n_slots; st->slot_bytes = L.slot_bytes; st->stash = st->ws + L.off_stash; st->bs = L.bs;
+  st->work_slot = cfg->checkpoint ? st->ws + L.work_slot : nullptr;
+  st->ck_in = L.ck_in; st->ck_tgt = L.ck_tgt;
+  st->sc_dmask = cfg->dropout_p > 0.f ? st->ws + L.sc_dmask : nullptr;
+  st->sc_loss = (float*)(st->ws + L.sc_loss);
   st->off_tok = L.off_tok; st->off_xf_in = L.off_xf_in; st->off_xf = L.off_xf; st->off_meanf = L.off_meanf;
   st->off_rstdf = L.off_rstdf; st->off_z = L.off_z;
   st->sc_proj = st->ws + L.sc_proj; st->sc_emb = st->ws + L.sc_emb; st->sc_dxa = st->ws + L.sc_dxa;
@@ -226,9 +258,31 @@ int paci_stage_create(const paci_stage_config* cfg, void* dev_ws, size_t ws_byte
   st->sc_attn = (float*)(st->ws + L.sc_attn);
   st->version = 0; st->q = 0; st->c = 0; st->n_forwards = 0;
   st->log.assign(LOG_CAP, {-1, -1, false});
+  // pointer tables: no string building or hashing on the issuing thread after this point
+  auto ref = [&](const std::string& name) {
+    const TensorInfo& t = st->tensors[st->index.at(name)];
+    Wref r;
+    r.w = st->W + t.offset;
+    r.g = st->G + t.offset;
+    r.wc = st->Wb ? (const void*)(st->Wb + t.offset) : (const void*)(st->W + t.offset);
+    return r;
+  };
+  st->bw.resize(st->L);
+  for (int l = 0; l < st->L; ++l) {
+    const std::string p = "h." + std::to_string(l) + ".";
+    st->bw[l] = BlockW{ref(p + "ln1.g"), ref(p + "ln1.b"), ref(p + "attn.wqkv"), ref(p + "attn.bqkv"), ref(p + "attn.wo"),
+                       ref(p + "attn.bo"), ref(p + "ln2.g"),  ref(p + "ln2.b"),  ref(p + "mlp.w1"),    ref(p + "mlp.b1"),
+                       ref(p + "mlp.w2"),  ref(p + "mlp.b2")};
+  }
+  st->wte = st->wpe = st->lnfg = st->lnfb = st->head = Wref{nullptr, nullptr, nullptr};
+  if (cfg->has_embedding) { st->wte = ref("wte"); st->wpe = ref("wpe"); }
+  if (cfg->has_head) {
+    st->lnfg = ref("lnf.g"); st->lnfb = ref("lnf.b");
+    st->head = ref(cfg->has_embedding ? "wte" : "head.w");
+  }
   cudaStream_t cs = (cudaStream_t)stream;
   cudaError_t e = cudaMemsetAsync(st->Mo, 0, (L.off_Wb - L.off_M), cs);          // m, v, G
-  if (e == cudaSuccess) e = cudaMemsetAsync(st->dev_version, 0, 8 + (size_t)LOG_CAP * 16, cs);
+  if (e == cudaSuccess) e = cudaMemsetAsync(st->dev_version, 0, 16 + (size_t)LOG_CAP * 16, cs);
   if (e != cudaSuccess) {
     delete st;
     return fail(PACI_ECUDA, "memset: %s", cudaGetErrorString(e));
@@ -320,90 +374,84 @@ int paci_stage_device_stamps(paci_stage_t* st, int64_t mb_id, int64_t* vF, int64
 // ------------------------------------------------------------------------------------------------
 namespace paci {
 
-struct Wref {   // pointers to one tensor in every group
-  float* w; float* g; const void* wc;   // master, grad accumulator, compute-dtype weights (shadow or master)
-};
-static Wref wref(paci_stage* st, const std::string& name) {
-  const TensorInfo& t = st->tensors[st->index.at(name)];
-  Wref r;
-  r.w = st->W + t.offset;
-  r.g = st->G + t.offset;
-  r.wc = st->Wb ? (const void*)(st->Wb + t.offset) : (const void*)(st->W + t.offset);
-  return r;
-}
-
 #define RC(expr) do { int rc__ = (expr); if (rc__ != PACI_OK) return rc__; } while (0)
 
-static int forward_impl(paci_stage* st, char* slot, const void* in, const int32_t* targets, void* out,
-                        cudaStream_t cs) {
-  const int dt = st->dtype, M = st->M, D = st->D;
+// dropout sites (R23): 0 = embedding output, 1 + 2l = attention branch of block l, 2 + 2l = its MLP branch
+static inline int site_attn(int l) { return 1 + 2 * l; }
+static inline int site_mlp(int l) { return 2 + 2 * l; }
+
+// One forward of the stage over n_seq sequences into the activation set `act` (a stash slot, or the checkpoint
+// mode's work slot).  x: int32 tokens [n_seq, T] (already inside the stash) if has_embedding, else h [n_seq, T, D].
+// out: h [n_seq, T, D] (may be NULL: recomputation does not need it), or float loss[1] on the head stage.
+static int forward_impl(paci_stage* st, char* act, const void* x, const int32_t* targets, void* out, int n_seq,
+                        int64_t mb_id, cudaStream_t cs) {
+  const int dt = st->dtype, M = n_seq * st->T, D = st->D;
+  const float pd = st->cfg.dropout_p;
+  const uint64_t seed = st->cfg.dropout_seed;
   const void* xa;           // residual stream = xa (+ xb)
   const void* xb = nullptr;
   if (st->cfg.has_embedding) {
-    int32_t* tok = (int32_t*)(slot + st->off_tok);
-    PACI_CUDA_OK(cudaMemcpyAsync(tok, in, (size_t)M * 4, cudaMemcpyDeviceToDevice, cs));
-    Wref wte = wref(st, "wte"), wpe = wref(st, "wpe");
-    RC(embed_fwd(dt, st->mu, st->T, D, tok, wte.w, wpe.w, st->sc_emb, cs));
+    RC(embed_fwd(dt, n_seq, st->T, D, (const int32_t*)x, st->wte.w, st->wpe.w, st->sc_emb, st->V, st->dev_err, cs));
+    if (pd > 0.f) RC(dropout(dt, (size_t)M * D, st->sc_emb, st->sc_emb, pd, seed, mb_id, 0, cs));
     xa = st->sc_emb;
   } else {
-    xa = in;
+    xa = x;
   }
   for (int l = 0; l < st->L; ++l) {
     const BlockStash& b = st->bs[l];
-    const std::string p = "h." + std::to_string(l) + ".";
-    Wref ln1g = wref(st, p + "ln1.g"), ln1b = wref(st, p + "ln1.b"), wqkv = wref(st, p + "attn.wqkv"),
-         bqkv = wref(st, p + "attn.bqkv"), wo = wref(st, p + "attn.wo"), bo = wref(st, p + "attn.bo"),
-         ln2g = wref(st, p + "ln2.g"), ln2b = wref(st, p + "ln2.b"), w1 = wref(st, p + "mlp.w1"),
-         b1 = wref(st, p + "mlp.b1"), w2 = wref(st, p + "mlp.w2"), b2 = wref(st, p + "mlp.b2");
+    const BlockW& w = st->bw[l];
     // a2: x_in = xa + xb (stashed), y1 = LN1(x_in)
-    RC(ln_fwd(dt, M, D, xa, xb, ln1g.w, ln1b.w, slot + b.x_in, slot + b.y1, (float*)(slot + b.mean1),
-              (float*)(slot + b.rstd1), cs));
+    RC(ln_fwd(dt, M, D, xa, xb, w.ln1g.w, w.ln1b.w, act + b.x_in, act + b.y1, (float*)(act + b.mean1),
+              (float*)(act + b.rstd1), cs));
     // a3: qkv = y1 Wqkv^T + b
-    RC(gemm(dt, 0, M, 3 * D, D, slot + b.y1, D, wqkv.wc, D, bqkv.w, slot + b.qkv, 3 * D, 0, cs));
+    RC(gemm(dt, 0, M, 3 * D, D, act + b.y1, D, w.wqkv.wc, D, w.bqkv.w, act + b.qkv, 3 * D, 0, cs));
     // a4: causal attention
-    RC(attention_fwd(dt, st->mu, st->T, st->H, st->dh, slot + b.qkv, slot + b.o, (float*)(slot + b.lse), cs));
+    RC(attention_fwd(dt, n_seq, st->T, st->H, st->dh, act + b.qkv, act + b.o, (float*)(act + b.lse), cs));
     // a5: a = o Wo^T + b
-    RC(gemm(dt, 0, M, D, D, slot + b.o, D, wo.wc, D, bo.w, st->sc_proj, D, 0, cs));
+    RC(gemm(dt, 0, M, D, D, act + b.o, D, w.wo.wc, D, w.bo.w, st->sc_proj, D, 0, cs));
+    if (pd > 0.f) RC(dropout(dt, (size_t)M * D, st->sc_proj, st->sc_proj, pd, seed, mb_id, site_attn(l), cs));
     // a6: x1 = x_in + a (stashed), y2 = LN2(x1)
-    RC(ln_fwd(dt, M, D, slot + b.x_in, st->sc_proj, ln2g.w, ln2b.w, slot + b.x1, slot + b.y2,
-              (float*)(slot + b.mean2), (float*)(slot + b.rstd2), cs));
-    // a7: p = y2 W1^T + b1 ; a8: g = gelu(p)
-    // gemm_bias_gelu (GELU in the GEMM epilogue) exists and is parity-clean, but with 4 epilogue warps its extra
-    // epilogue work costs the MLP-up GEMM what the separate 4.7 TB/s kernel costs (measured: 0 net): not used yet.
-    RC(gemm(dt, 0, M, 4 * D, D, slot + b.y2, D, w1.wc, D, b1.w, slot + b.p, 4 * D, 0, cs));
-    RC(gelu_fwd(dt, (size_t)M * 4 * D, slot + b.p, slot + b.g, cs));
+    RC(ln_fwd(dt, M, D, act + b.x_in, st->sc_proj, w.ln2g.w, w.ln2b.w, act + b.x1, act + b.y2,
+              (float*)(act + b.mean2), (float*)(act + b.rstd2), cs));
+    // a7 + a8: p = y2 W1^T + b1 (stashed: backward needs gelu'(p)) and g = gelu(p), one launch in bf16 mode (the
+    // activation is computed in the GEMM epilogue and leaves through a second TMA store)
+    RC(gemm_bias_gelu(dt, M, 4 * D, D, act + b.y2, D, w.w1.wc, D, w.b1.w, act + b.p, act + b.g, 4 * D, cs));
     // a9: m = g W2^T + b2 ; the residual add is fused into the next LayerNorm
-    RC(gemm(dt, 0, M, D, 4 * D, slot + b.g, 4 * D, w2.wc, 4 * D, b2.w, st->sc_proj, D, 0, cs));
-    xa = slot + b.x1;
+    RC(gemm(dt, 0, M, D, 4 * D, act + b.g, 4 * D, w.w2.wc, 4 * D, w.b2.w, st->sc_proj, D, 0, cs));
+    if (pd > 0.f) RC(dropout(dt, (size_t)M * D, st->sc_proj, st->sc_proj, pd, seed, mb_id, site_mlp(l), cs));
+    xa = act + b.x1;
     xb = st->sc_proj;
   }
-  if (!st->cfg.has_head) return add_vec(dt, (size_t)M * D, xa, xb, out, cs);
-  // a10: z = LN_f(x) Whead^T ; a11: loss and dz in place
-  Wref lnfg = wref(st, "lnf.g"), lnfb = wref(st, "lnf.b");
-  Wref head = wref(st, st->cfg.has_embedding ? "wte" : "head.w");
-  RC(ln_fwd(dt, M, D, xa, xb, lnfg.w, lnfb.w, slot + st->off_xf_in, slot + st->off_xf,
-            (float*)(slot + st->off_meanf), (float*)(slot + st->off_rstdf), cs));
-  RC(gemm(dt, 0, M, st->V, D, slot + st->off_xf, D, head.wc, D, nullptr, slot + st->off_z, st->Vpad, 0, cs));
+  if (!st->cfg.has_head) return out != nullptr ? add_vec(dt, (size_t)M * D, xa, xb, out, cs) : PACI_OK;
+  // a10: z = LN_f(x) Whead^T ; a11: loss (mean over THIS micro-batch's tokens, R22) and dz in place
+  RC(ln_fwd(dt, M, D, xa, xb, st->lnfg.w, st->lnfb.w, act + st->off_xf_in, act + st->off_xf,
+            (float*)(act + st->off_meanf), (float*)(act + st->off_rstdf), cs));
+  RC(gemm(dt, 0, M, st->V, D, act + st->off_xf, D, st->head.wc, D, nullptr, act + st->off_z, st->Vpad, 0, cs));
   PACI_CUDA_OK(cudaMemsetAsync(out, 0, sizeof(float), cs));
-  return softmax_ce(dt, M, st->V, st->Vpad, slot + st->off_z, targets, (float*)out, cs);
+  return softmax_ce(dt, M, st->V, st->Vpad, act + st->off_z, targets, (float*)out, st->dev_err, cs);
 }
 
-static int backward_impl(paci_stage* st, char* slot, const void* dout, void* din, cudaStream_t cs) {
-  const int dt = st->dtype, M = st->M, D = st->D;
+// Backward over the activation set `act` with the stage's CURRENT parameters (Eq. 1).  tok: the stashed
+// int32 tokens (embedding stage).
+static int backward_impl(paci_stage* st, char* act, const int32_t* tok, const void* dout, void* din, int n_seq,
+                         int64_t mb_id, cudaStream_t cs) {
+  const int dt = st->dtype, M = n_seq * st->T, D = st->D;
+  const float pd = st->cfg.dropout_p;
+  const uint64_t seed = st->cfg.dropout_seed;
+  const bool drop = pd > 0.f;
   const void* dcur;                     // grad wrt the residual stream at the current depth
-  float* pending_b2 = nullptr;          // G of the bias whose gradient is colsum(dcur)
-  if (st->L > 0) pending_b2 = wref(st, "h." + std::to_string(st->L - 1) + ".mlp.b2").g;
+  // no dropout: colsum(dcur) IS the gradient of the last block's b2 and is fused into the producer of dcur (a15).
+  // dropout: the branch gradient is mask o dcur / (1 - p), so the bias gradients are column sums of the masked copy.
+  float* pending_b2 = (!drop && st->L > 0) ? st->bw[st->L - 1].b2.g : nullptr;
   char* pp[2] = {st->sc_dxa, st->sc_dxb};
   int flip = 0;
   if (st->cfg.has_head) {
-    Wref lnfg = wref(st, "lnf.g"), lnfb = wref(st, "lnf.b");
-    Wref head = wref(st, st->cfg.has_embedding ? "wte" : "head.w");
     // a12: dxf = dz Whead (current weights, Eq. 1); G_head += dz^T xf (beta = 1 epilogue)
-    RC(gemm(dt, 1, M, D, st->V, slot + st->off_z, st->Vpad, head.wc, D, nullptr, st->sc_dD, D, 0, cs));
-    RC(gemm(dt, 2, st->V, D, M, slot + st->off_z, st->Vpad, slot + st->off_xf, D, nullptr, head.g, D, 1, cs));
+    RC(gemm(dt, 1, M, D, st->V, act + st->off_z, st->Vpad, st->head.wc, D, nullptr, st->sc_dD, D, 0, cs));
+    RC(gemm(dt, 2, st->V, D, M, act + st->off_z, st->Vpad, act + st->off_xf, D, nullptr, st->head.g, D, 1, cs));
     void* dst = (st->L == 0 && !st->cfg.has_embedding) ? din : (void*)pp[flip];
-    RC(ln_bwd(dt, M, D, st->sc_dD, slot + st->off_xf_in, (float*)(slot + st->off_meanf),
-              (float*)(slot + st->off_rstdf), lnfg.w, nullptr, dst, lnfg.g, lnfb.g, pending_b2, cs));
+    RC(ln_bwd(dt, M, D, st->sc_dD, act + st->off_xf_in, (float*)(act + st->off_meanf),
+              (float*)(act + st->off_rstdf), st->lnfg.w, nullptr, dst, st->lnfg.g, st->lnfb.g, pending_b2, cs));
     pending_b2 = nullptr;
     dcur = dst;
     flip ^= 1;
@@ -412,47 +460,57 @@ static int backward_impl(paci_stage* st, char* slot, const void* dout, void* din
   }
   for (int l = st->L - 1; l >= 0; --l) {
     const BlockStash& b = st->bs[l];
-    const std::string p = "h." + std::to_string(l) + ".";
-    Wref ln1g = wref(st, p + "ln1.g"), ln1b = wref(st, p + "ln1.b"), wqkv = wref(st, p + "attn.wqkv"),
-         bqkv = wref(st, p + "attn.bqkv"), wo = wref(st, p + "attn.wo"), bo = wref(st, p + "attn.bo"),
-         ln2g = wref(st, p + "ln2.g"), ln2b = wref(st, p + "ln2.b"), w1 = wref(st, p + "mlp.w1"),
-         b1 = wref(st, p + "mlp.b1"), w2 = wref(st, p + "mlp.w2");
-    if (pending_b2) {   // a15: only when dcur came from outside the stage (no producer to fuse into)
+    const BlockW& w = st->bw[l];
+    const void* dm = dcur;              // grad wrt the MLP branch output
+    if (drop) {
+      RC(dropout(dt, (size_t)M * D, dcur, st->sc_dmask, pd, seed, mb_id, site_mlp(l), cs));
+      RC(colsum(dt, M, D, st->sc_dmask, w.b2.g, cs));
+      dm = st->sc_dmask;
+    } else if (pending_b2) {   // a15: only when dcur came from outside the stage (no producer to fuse into)
       RC(colsum(dt, M, D, dcur, pending_b2, cs));
       pending_b2 = nullptr;
     }
-    // MLP-down: dg = dx2 W2 ; G_W2 += dx2^T g
-    RC(gemm(dt, 1, M, 4 * D, D, dcur, D, w2.wc, 4 * D, nullptr, st->sc_d4, 4 * D, 0, cs));
-    RC(gemm(dt, 2, D, 4 * D, M, dcur, D, slot + b.g, 4 * D, nullptr, w2.g, 4 * D, 1, cs));
+    // MLP-down: dg = dm W2 ; G_W2 += dm^T g
+    RC(gemm(dt, 1, M, 4 * D, D, dm, D, w.w2.wc, 4 * D, nullptr, st->sc_d4, 4 * D, 0, cs));
+    RC(gemm(dt, 2, D, 4 * D, M, dm, D, act + b.g, 4 * D, nullptr, w.w2.g, 4 * D, 1, cs));
     // a16: dp = dg * gelu'(p) in place ; G_b1 += colsum(dp)
-    RC(gelu_bwd(dt, M, 4 * D, st->sc_d4, slot + b.p, st->sc_d4, b1.g, cs));
+    RC(gelu_bwd(dt, M, 4 * D, st->sc_d4, act + b.p, st->sc_d4, w.b1.g, cs));
     // MLP-up: dy2 = dp W1 ; G_W1 += dp^T y2
-    RC(gemm(dt, 1, M, D, 4 * D, st->sc_d4, 4 * D, w1.wc, D, nullptr, st->sc_dD, D, 0, cs));
-    RC(gemm(dt, 2, 4 * D, D, M, st->sc_d4, 4 * D, slot + b.y2, D, nullptr, w1.g, D, 1, cs));
-    // a18: dx1 = dx2 + LN2bwd(dy2) ; G_ln2 ; G_bo += colsum(dx1)
-    RC(ln_bwd(dt, M, D, st->sc_dD, slot + b.x1, (float*)(slot + b.mean2), (float*)(slot + b.rstd2), ln2g.w, dcur,
-              st->sc_dx1, ln2g.g, ln2b.g, bo.g, cs));
-    // out-proj: do = dx1 Wo ; G_Wo += dx1^T o
-    RC(gemm(dt, 1, M, D, D, st->sc_dx1, D, wo.wc, D, nullptr, st->sc_dD2, D, 0, cs));
-    RC(gemm(dt, 2, D, D, M, st->sc_dx1, D, slot + b.o, D, nullptr, wo.g, D, 1, cs));
+    RC(gemm(dt, 1, M, D, 4 * D, st->sc_d4, 4 * D, w.w1.wc, D, nullptr, st->sc_dD, D, 0, cs));
+    RC(gemm(dt, 2, 4 * D, D, M, st->sc_d4, 4 * D, act + b.y2, D, nullptr, w.w1.g, D, 1, cs));
+    // a18: dx1 = dcur + LN2bwd(dy2) ; G_ln2 ; G_bo += colsum(dx1) (no dropout)
+    RC(ln_bwd(dt, M, D, st->sc_dD, act + b.x1, (float*)(act + b.mean2), (float*)(act + b.rstd2), w.ln2g.w, dcur,
+              st->sc_dx1, w.ln2g.g, w.ln2b.g, drop ? nullptr : w.bo.g, cs));
+    const void* da = st->sc_dx1;        // grad wrt the attention branch output
+    if (drop) {
+      RC(dropout(dt, (size_t)M * D, st->sc_dx1, st->sc_dmask, pd, seed, mb_id, site_attn(l), cs));
+      RC(colsum(dt, M, D, st->sc_dmask, w.bo.g, cs));
+      da = st->sc_dmask;
+    }
+    // out-proj: do = da Wo ; G_Wo += da^T o
+    RC(gemm(dt, 1, M, D, D, da, D, w.wo.wc, D, nullptr, st->sc_dD2, D, 0, cs));
+    RC(gemm(dt, 2, D, D, M, da, D, act + b.o, D, nullptr, w.wo.g, D, 1, cs));
     // a17: attention backward
-    RC(attention_bwd(dt, st->mu, st->T, st->H, st->dh, st->sc_dD2, slot + b.qkv, slot + b.o,
-                     (float*)(slot + b.lse), st->sc_dqkv, st->sc_attn, bqkv.g, cs));   // + G_bqkv (a15)
+    RC(attention_bwd(dt, n_seq, st->T, st->H, st->dh, st->sc_dD2, act + b.qkv, act + b.o,
+                     (float*)(act + b.lse), st->sc_dqkv, st->sc_attn, w.bqkv.g, cs));   // + G_bqkv (a15)
     // QKV: dy1 = dqkv Wqkv ; G_Wqkv += dqkv^T y1
-    RC(gemm(dt, 1, M, D, 3 * D, st->sc_dqkv, 3 * D, wqkv.wc, D, nullptr, st->sc_dD, D, 0, cs));
-    RC(gemm(dt, 2, 3 * D, D, M, st->sc_dqkv, 3 * D, slot + b.y1, D, nullptr, wqkv.g, D, 1, cs));
-    // a18: dx = dx1 + LN1bwd(dy1) ; G_ln1 ; colsum(dx) is the previous block's G_b2
-    float* gcol = l > 0 ? wref(st, "h." + std::to_string(l - 1) + ".mlp.b2").g : nullptr;
+    RC(gemm(dt, 1, M, D, 3 * D, st->sc_dqkv, 3 * D, w.wqkv.wc, D, nullptr, st->sc_dD, D, 0, cs));
+    RC(gemm(dt, 2, 3 * D, D, M, st->sc_dqkv, 3 * D, act + b.y1, D, nullptr, w.wqkv.g, D, 1, cs));
+    // a18: dx = dx1 + LN1bwd(dy1) ; G_ln1 ; colsum(dx) is the previous block's G_b2 (no dropout)
+    float* gcol = (!drop && l > 0) ? st->bw[l - 1].b2.g : nullptr;
     void* dst = (l == 0 && !st->cfg.has_embedding) ? din : (void*)pp[flip];
-    RC(ln_bwd(dt, M, D, st->sc_dD, slot + b.x_in, (float*)(slot + b.mean1), (float*)(slot + b.rstd1), ln1g.w,
-              st->sc_dx1, dst, ln1g.g, ln1b.g, gcol, cs));
+    RC(ln_bwd(dt, M, D, st->sc_dD, act + b.x_in, (float*)(act + b.mean1), (float*)(act + b.rstd1), w.ln1g.w,
+              st->sc_dx1, dst, w.ln1g.g, w.ln1b.g, gcol, cs));
     dcur = dst;
     flip ^= 1;
   }
   if (st->cfg.has_embedding) {
-    Wref wte = wref(st, "wte"), wpe = wref(st, "wpe");
+    if (drop) {
+      RC(dropout(dt, (size_t)M * D, dcur, st->sc_dmask, pd, seed, mb_id, 0, cs));
+      dcur = st->sc_dmask;
+    }
     // a19
-    return embed_bwd(dt, st->mu, st->T, D, (const int32_t*)(slot + st->off_tok), dcur, wte.g, wpe.g, cs);
+    return embed_bwd(dt, n_seq, st->T, D, tok, dcur, st->wte.g, st->wpe.g, st->V, cs);
   }
   if (st->L == 0 && !st->cfg.has_head) return add_vec(dt, (size_t)M * D, dcur, nullptr, din, cs);
   return PACI_OK;
@@ -462,9 +520,10 @@ static int backward_impl(paci_stage* st, char* slot, const void* dout, void* din
 
 extern "C" {
 
-int paci_forward(paci_stage_t* st, int64_t mb_id, const void* in, const int32_t* targets, void* out,
-                 void* stream) {
+int paci_forward_var(paci_stage_t* st, int64_t mb_id, int32_t n_seq, const void* in, const int32_t* targets,
+                     void* out, void* stream) {
   if (!st || !in || !out) return fail(PACI_EINVAL, "null pointer");
+  if (n_seq < 1 || n_seq > st->mu) return fail(PACI_EINVAL, "n_seq %d outside [1, micro_batch = %d]", n_seq, st->mu);
   if (st->cfg.has_head && !targets) return fail(PACI_EINVAL, "head stage needs targets");
   if (st->c == st->k) return fail(PACI_ESTATE, "update pending: call paci_maybe_step first");
   for (const auto& u : st->fifo)
@@ -475,17 +534,40 @@ int paci_forward(paci_stage_t* st, int64_t mb_id, const void* in, const int32_t*
   const int slot_i = (int)(st->n_forwards % st->n_slots);
   const int log_idx = (int)(st->n_forwards % LOG_CAP);
   char* slot = st->stash + (size_t)slot_i * st->slot_bytes;
+  const bool ck = st->cfg.checkpoint != 0;
+  const size_t M = (size_t)n_seq * st->T;
   int rc = stamp_version(st->dev_version, st->dev_stamps + 2 * (size_t)log_idx, cs);
-  if (rc == PACI_OK) rc = forward_impl(st, slot, in, targets, out, cs);
+  if (rc != PACI_OK) return rc;
+  // what backward needs of the stage INPUT goes into the stash: the tokens (embedding scatter-add), and in
+  // checkpoint mode the whole input and the targets (the recomputation starts from them)
+  const void* x = in;
+  if (st->cfg.has_embedding) {
+    int32_t* tok = (int32_t*)(slot + (ck ? st->ck_in : st->off_tok));
+    PACI_CUDA_OK(cudaMemcpyAsync(tok, in, M * 4, cudaMemcpyDeviceToDevice, cs));
+    x = tok;
+  } else if (ck) {
+    PACI_CUDA_OK(cudaMemcpyAsync(slot + st->ck_in, in, M * st->D * st->esz, cudaMemcpyDeviceToDevice, cs));
+  }
+  if (ck && st->cfg.has_head)
+    PACI_CUDA_OK(cudaMemcpyAsync(slot + st->ck_tgt, targets, M * 4, cudaMemcpyDeviceToDevice, cs));
+  rc = forward_impl(st, ck ? st->work_slot : slot, x, targets, out, n_seq, mb_id, cs);
   if (rc != PACI_OK) return rc;
   // bookkeeping (Alg. 1 line 9): t^F = version, q += 1
-  if (st->log[log_idx].mb >= 0) st->log_of.erase(st->log[log_idx].mb);
+  const int64_t old = st->log[log_idx].mb;
+  auto it = st->log_of.find(old);
+  if (it != st->log_of.end() && it->second == log_idx) st->log_of.erase(it);   // only if it still maps to THIS entry
   st->log[log_idx] = {mb_id, -1, false};
   st->log_of[mb_id] = log_idx;
-  st->fifo.push_back({mb_id, slot_i, st->version, log_idx});
+  st->fifo.push_back({mb_id, slot_i, st->version, log_idx, n_seq});
   st->q += 1;
   st->n_forwards += 1;
   return PACI_OK;
+}
+
+int paci_forward(paci_stage_t* st, int64_t mb_id, const void* in, const int32_t* targets, void* out,
+                 void* stream) {
+  if (!st) return fail(PACI_EINVAL, "null pointer");
+  return paci_forward_var(st, mb_id, st->mu, in, targets, out, stream);
 }
 
 int paci_backward(paci_stage_t* st, int64_t mb_id, const void* dout, void* din, void* stream) {
@@ -501,7 +583,17 @@ int paci_backward(paci_stage_t* st, int64_t mb_id, const void* dout, void* din, 
   cudaStream_t cs = (cudaStream_t)stream;
   char* slot = st->stash + (size_t)u.slot * st->slot_bytes;
   int rc = stamp_version(st->dev_version, st->dev_stamps + 2 * (size_t)u.log_idx + 1, cs);
-  if (rc == PACI_OK) rc = backward_impl(st, slot, dout, din, cs);
+  if (rc != PACI_OK) return rc;
+  if (st->cfg.checkpoint) {
+    // "those activations are instead recomputed under the current parameter version before differentiation"
+    const void* x = slot + st->ck_in;
+    rc = forward_impl(st, st->work_slot, x, (const int32_t*)(slot + st->ck_tgt), st->cfg.has_head ? st->sc_loss : nullptr,
+                      u.n_seq, mb_id, cs);
+    if (rc == PACI_OK)
+      rc = backward_impl(st, st->work_slot, (const int32_t*)x, dout, din, u.n_seq, mb_id, cs);
+  } else {
+    rc = backward_impl(st, slot, (const int32_t*)(slot + st->off_tok), dout, din, u.n_seq, mb_id, cs);
+  }
   if (rc != PACI_OK) return rc;
   // Eq. 8: Delta = t^B - t^F, read before line 16's test; lines 14-15: c += 1, q -= 1
   st->log[u.log_idx].delta = (int32_t)(st->version - u.vF);
@@ -522,6 +614,38 @@ int paci_maybe_step(paci_stage_t* st, float lr, void* stream) {
   st->version += 1;                 // lines 17-18
   st->c = 0;
   return 1;
+}
+
+int paci_stage_set_state(paci_stage_t* st, int64_t version, int32_t window_count, void* stream) {
+  if (!st) return fail(PACI_EINVAL, "null stage");
+  if (version < 0 || window_count < 0 || window_count >= st->k)
+    return fail(PACI_EINVAL, "set_state: version %lld, window_count %d (k = %d)", (long long)version, window_count, st->k);
+  if (st->q != 0) return fail(PACI_ESTATE, "set_state with %d unresolved forwards", st->q);
+  cudaStream_t cs = (cudaStream_t)stream;
+  PACI_CUDA_OK(cudaMemcpyAsync(st->dev_version, &version, 8, cudaMemcpyHostToDevice, cs));
+  PACI_CUDA_OK(cudaStreamSynchronize(cs));
+  st->version = version;
+  st->c = window_count;
+  return PACI_OK;
+}
+
+int paci_stage_check(paci_stage_t* st, void* stream) {
+  if (!st) return fail(PACI_EINVAL, "null stage");
+  cudaStream_t cs = (cudaStream_t)stream;
+  int64_t e = 0;
+  PACI_CUDA_OK(cudaMemcpyAsync(&e, st->dev_err, 8, cudaMemcpyDeviceToHost, cs));
+  PACI_CUDA_OK(cudaStreamSynchronize(cs));
+  if (e == 0) return PACI_OK;
+  PACI_CUDA_OK(cudaMemsetAsync(st->dev_err, 0, 8, cs));
+  PACI_CUDA_OK(cudaStreamSynchronize(cs));
+  return fail(PACI_EINVAL, "stage %d: a token or target id was outside [0, %d) (clamped on the device)", st->s, st->V);
+}
+
+float paci_lr_schedule(int64_t step, int64_t total_steps, int64_t warmup_steps, float peak, float final_frac) {
+  if (warmup_steps > 0 && step < warmup_steps) return peak * (float)((double)(step + 1) / (double)warmup_steps);
+  if (step >= total_steps || total_steps <= warmup_steps) return peak * final_frac;
+  const double prog = (double)(step - warmup_steps) / (double)(total_steps - warmup_steps);
+  return (float)((double)peak * ((double)final_frac + (1.0 - (double)final_frac) * 0.5 * (1.0 + std::cos(3.14159265358979323846 * prog))));
 }
 
 }  // extern "C"
