@@ -227,6 +227,20 @@ int paci_pipeline_run_var(paci_pipeline_t* p, const int32_t* tokens, int32_t tok
                           int64_t n_microbatches, const int32_t* n_seq, int32_t mode, float lr,
                           const float* lr_by_update, int64_t n_updates, void* stream, paci_run_report* rep);
 
+/* ---- memory-constrained pipeline partitioning (App. D.5, Eq. 12-15; host arithmetic only) ---------- */
+/* Splits n_layers sequential layers into n_stages contiguous groups minimising the slowest stage's time
+ * max_j sum t_l subject to  sum s_l + w_j sum a_l <= budget  for every stage j, w_j = n_stages - j + 1 in-flight
+ * micro-batches (Eq. 12-13; "the first stage carries N microbatches, the last carries one"), by the paper's
+ * two-pass dynamic program (Eq. 15; infeasibility fallback: minimise the worst overshoot, ties by the maximum stage
+ * time).
+ *   t, s, a   HOST double [n_layers]: forward time, static bytes (parameters, gradients, optimizer state) and
+ *             activation bytes per micro-batch of each layer (any consistent units)
+ *   cuts      HOST int32 [n_stages + 1], out: 0 = c_0 < c_1 < ... < c_N = n_layers
+ *   max_stage_time, max_overshoot   HOST, out (may be NULL)
+ * Returns 0 (feasible: Eq. 13's optimum), 1 (budget infeasible: the fallback's partition), or PACI_EINVAL. */
+int paci_partition(int32_t n_layers, int32_t n_stages, const double* t, const double* s, const double* a,
+                   double budget, int32_t* cuts, double* max_stage_time, double* max_overshoot);
+
 /* ---- op-level entry points (kernel parity tests and per-kernel roofline measurements) ------ */
 /* All pointers DEVICE.  dtype = PACI_FP32 | PACI_BF16 selects the activation type T below. */
 

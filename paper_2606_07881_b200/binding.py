@@ -71,6 +71,8 @@ SIGNATURES = {
     "paci_pipeline_run": (_i, [_vp, _vp, C.c_int32, _i64, C.c_int32, _f, _vp, C.POINTER(RunReport)]),
     "paci_pipeline_run_var": (_i, [_vp, _vp, C.c_int32, _i64, _vp, C.c_int32, _f, _vp, _i64, _vp,
                                    C.POINTER(RunReport)]),
+    "paci_partition": (_i, [C.c_int32, C.c_int32, _vp, _vp, _vp, C.c_double, _vp, C.POINTER(C.c_double),
+                            C.POINTER(C.c_double)]),
     "paci_op_gemm": (_i, [_i, _i, _i, _i, _i, _vp, _i, _vp, _i, _vp, _vp, _i, _i, _vp]),
     "paci_op_gemm_bias_gelu": (_i, [_i, _i, _i, _i, _vp, _i, _vp, _i, _vp, _vp, _vp, _i, _vp]),
     "paci_op_layernorm_fwd": (_i, [_i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -152,6 +154,16 @@ def gemm_last_plan() -> dict:
     out = (C.c_int32 * 6)()
     lib.paci_gemm_last_plan(out)
     return dict(zip(("cta_group", "block_n", "splits", "range_mode", "grid", "tiles"), list(out)))
+
+
+def partition(t, s, a, n_stages, budget) -> dict:
+    """App. D.5: cut points of the memory-constrained min-max partition."""
+    t, s, a = (np.ascontiguousarray(v, dtype=np.float64) for v in (t, s, a))
+    cuts = np.zeros(n_stages + 1, np.int32)
+    mt, mo = C.c_double(), C.c_double()
+    rc = check(lib.paci_partition(len(t), n_stages, t.ctypes.data, s.ctypes.data, a.ctypes.data, float(budget),
+                                  cuts.ctypes.data, C.byref(mt), C.byref(mo)), "paci_partition")
+    return dict(cuts=cuts.tolist(), max_time=mt.value, max_overshoot=mo.value, fallback=bool(rc))
 
 
 def lr_schedule(step, total_steps, warmup_steps, peak, final_frac=0.1) -> float:

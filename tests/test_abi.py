@@ -69,3 +69,24 @@ def test_workspace_holds_one_parameter_copy_and_S_minus_s_stash_slots(pb):
 def test_missing_library_fails_loudly(pb):
     with pytest.raises(ImportError, match="no CPU fallback"):
         pb.load_library("/nonexistent/libpaci.so")
+
+
+def test_lr_schedule_host_function_matches_oracle(pb):
+    """paci_lr_schedule (1% linear warm-up, cosine to 10% of the peak) is pure host arithmetic: every step of
+    a 1000-update schedule against oracle/lr.py."""
+    from oracle import lr as olr
+    for peak in (3e-4, 3 * 0.5 ** 0.5 * 1e-4):
+        for t in list(range(0, 30)) + list(range(30, 1100, 7)):
+            want = olr.lr_at(t, 1000, 10, peak)
+            assert abs(pb.lr_schedule(t, 1000, 10, peak) - want) <= 1e-7 * want, t
+
+
+def test_checkpoint_and_dropout_config_validation(pb):
+    ok = pb.make_config(0, 2, 1, 64, 4, 32, 2, 4, 256, pb.FP32, checkpoint=1, dropout_p=0.1, dropout_seed=5)
+    base = pb.make_config(0, 2, 1, 64, 4, 32, 2, 4, 256, pb.FP32)
+    assert 0 < pb.lib.paci_stage_workspace_bytes(C.byref(ok))
+    assert pb.lib.paci_stage_param_count(C.byref(ok)) == pb.lib.paci_stage_param_count(C.byref(base))   # one parameter copy
+    for bad in (pb.make_config(0, 2, 1, 64, 4, 32, 2, 4, 256, pb.FP32, checkpoint=2),
+                pb.make_config(0, 2, 1, 64, 4, 32, 2, 4, 256, pb.FP32, dropout_p=1.0),
+                pb.make_config(0, 2, 1, 128, 2, 64, 2, 4, 256, pb.BF16)):     # bf16: T % 128
+        assert pb.lib.paci_stage_workspace_bytes(C.byref(bad)) == 0

@@ -28,6 +28,11 @@ def _build(dtype, S, L, D, H, T, mu, V, k, seed=1234):
 # gradient error e (1e-5 fp32) a fraction ~e of the elements flips: rel-L2 ~ sqrt(e)*2*lr/rms(w) ~ 3e-4
 # at lr 1e-3, rms 0.02.  Gate: 1e-3 in fp32 mode (derived), 2e-2 in bf16 mode (BASELINE.json).
 WTOL = {pb.FP32: 1e-3, pb.BF16: 2e-2}
+# Gradient accumulators of the TAIL window are computed AFTER optimizer steps, i.e. under weights that already differ
+# from the oracle's by the sign-flip noise above, so in fp32 mode the first window's per-parameter gate (TOL = 1e-5) is
+# widened by the propagated weight error: a fraction ~1e-5 of the elements moved by 2 lr, which perturbs a gradient by a
+# few 1e-5 relative.  bf16: BASELINE.json's gate, 2e-2, unchanged.
+GTOL_TAIL = {pb.FP32: 4e-5, pb.BF16: 2e-2}
 
 
 def _compare(out, ref, stages, dtype, n, loss_tol, lr_bound=2e-3):
@@ -45,7 +50,7 @@ def _compare(out, ref, stages, dtype, n, loss_tol, lr_bound=2e-3):
             assert rel_l2(got, th) < WTOL[dtype], (s, name)
             G = ref["opt"][s].G[name]                            # tail window (n % k backwards) stays in G
             if np.any(G):
-                assert rel_l2(st.read(name, pb.GRAD_ACCUM), G) < 4 * TOL[dtype], (s, name)
+                assert rel_l2(st.read(name, pb.GRAD_ACCUM), G) < GTOL_TAIL[dtype], (s, name)
             else:
                 assert np.count_nonzero(st.read(name, pb.GRAD_ACCUM)) == 0
 
@@ -101,7 +106,7 @@ def test_flush_mode_matches_oracle_and_never_crosses():
 
 def test_bf16_pipeline_small():
     """bf16 mode, 3 stages: counts exact, loss / weights within the bf16 gates after two updates."""
-    V, D, H, T, mu, S, L, k, n = 1000, 128, 2, 64, 2, 3, 1, 2, 4
+    V, D, H, T, mu, S, L, k, n = 1000, 128, 2, 128, 2, 3, 1, 2, 4
     specs, params, stages = _build(pb.BF16, S, L, D, H, T, mu, V, k, seed=9)
     tok = synth.tokens(9, n, mu, T, V, "zipf")
     ref = opipe.run_pipeline(specs, params, tok, k, 3e-4)
