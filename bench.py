@@ -358,7 +358,7 @@ def run_ours(args, c, name):
             # this category's estimated share of the step: mean sampled duration x launches
             d["est_ms_per_step"] = round(e["sampled_ms"] / e["sampled"] * e["launches"] / args.steps, 3)
         cats[n] = d
-    g = [prof[n] for n in ("gemm_fwd", "gemm_dgrad", "gemm_wgrad")]
+    g = [prof[n] for n in ("gemm_fwd", "gemm_dgrad", "gemm_wgrad", "gemm_bwd_pair")]
     g_ms = sum(e["sampled_ms"] for e in g)
     g_flops = sum(e["sampled_flops"] for e in g)
     g_n = sum(e["sampled"] for e in g)

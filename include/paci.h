@@ -253,6 +253,12 @@ int paci_partition(int32_t n_layers, int32_t n_stages, const double* t, const do
  * PACI_BF16: all leading dimensions and pointers must be multiples of 8 elements / 16 bytes. */
 int paci_op_gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
                  const float* bias, void* C, int ldc, int out_f32_accum, void* stream);
+/* The backward pair of one linear layer y = x W^T (rows a13 + a14): G_W[N_out, K_in] += dy^T x (fp32, beta = 1, Alg. 1
+ * line 13) and dx[M, K_in] = dy W (the CURRENT W, Eq. 1).  dy [M, N_out], x [M, K_in], W [N_out, K_in], all row-major T
+ * with the given row strides.  PACI_BF16: ONE tcgen05 launch -- the dgrad's tiles are dealt round-robin over the CTA
+ * pairs and the wgrad's (tile, k-block) units are poured on top until every pair carries the same number of k-blocks. */
+int paci_op_gemm_backward_pair(int dtype, int M, int N_out, int K_in, const void* dy, int ld_dy, const void* x, int ld_x,
+                               const void* W, int ld_w, float* G_W, int ld_g, void* dx, int ld_dx, void* stream);
 /* MLP-up with the activation fused (rows a7 + a8):  C = A B^T + bias (the pre-activation, which backward needs)
  * and G = gelu(C), both [M, N] of T with row stride ldc, A[M,K], B[N,K] row-major.  PACI_BF16 on the tcgen05 path:
  * ONE launch, gelu of the rounded C is computed in the GEMM epilogue and leaves through a second TMA store;
@@ -306,11 +312,11 @@ int paci_op_adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float*
 
 /* ---- sampled kernel timing (bench.py "roofline") ----------------------------- */
 /* Categories, in order: gemm_fwd, gemm_dgrad, gemm_wgrad, attention_fwd, attention_bwd, layernorm_fwd,
- * layernorm_bwd, gelu_fwd, gelu_bwd, colsum, embedding, softmax_ce, adamw, other.  flops / bytes are
+ * layernorm_bwd, gelu_fwd, gelu_bwd, colsum, embedding, softmax_ce, adamw, other, gemm_bwd_pair.  flops / bytes are
  * the ALGORITHMIC work of the op, summed over every launch since
  * paci_profile_begin; every sample_stride-th launch is bracketed by CUDA events on the stream it is
  * launched on, and sampled_* sum those launches only (sampled_ms = their device time). */
-#define PACI_PROF_NCAT 14
+#define PACI_PROF_NCAT 15
 typedef struct paci_prof_entry {
   int64_t launches, sampled;
   double flops, bytes, sampled_flops, sampled_bytes, sampled_ms;

@@ -40,7 +40,7 @@ class ProfEntry(C.Structure):
         "flops", "bytes", "sampled_flops", "sampled_bytes", "sampled_ms")]
 
 
-PROF_NCAT = 14
+PROF_NCAT = 15
 
 # name -> (restype, argtypes); every symbol include/paci.h declares
 _vp, _i, _i64, _sz, _f = C.c_void_p, C.c_int, C.c_int64, C.c_size_t, C.c_float
@@ -74,6 +74,7 @@ SIGNATURES = {
     "paci_partition": (_i, [C.c_int32, C.c_int32, _vp, _vp, _vp, C.c_double, _vp, C.POINTER(C.c_double),
                             C.POINTER(C.c_double)]),
     "paci_op_gemm": (_i, [_i, _i, _i, _i, _i, _vp, _i, _vp, _i, _vp, _vp, _i, _i, _vp]),
+    "paci_op_gemm_backward_pair": (_i, [_i, _i, _i, _i, _vp, _i, _vp, _i, _vp, _i, _vp, _i, _vp, _i, _vp]),
     "paci_op_gemm_bias_gelu": (_i, [_i, _i, _i, _i, _vp, _i, _vp, _i, _vp, _vp, _vp, _i, _vp]),
     "paci_op_layernorm_fwd": (_i, [_i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_layernorm_bwd": (_i, [_i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),

@@ -129,7 +129,7 @@ int set_max_dynamic_smem(const void* func, int bytes);
 
 // ---------------------------------------------------------------- sampled kernel timing (prof.cu)
 enum ProfCat { PC_GEMM_FWD = 0, PC_GEMM_DGRAD, PC_GEMM_WGRAD, PC_ATTN_FWD, PC_ATTN_BWD, PC_LN_FWD, PC_LN_BWD,
-               PC_GELU_FWD, PC_GELU_BWD, PC_COLSUM, PC_EMBED, PC_SOFTMAX_CE, PC_ADAMW, PC_OTHER };
+               PC_GELU_FWD, PC_GELU_BWD, PC_COLSUM, PC_EMBED, PC_SOFTMAX_CE, PC_ADAMW, PC_OTHER, PC_GEMM_BWD_PAIR };
 struct ProfScope {   // counts the launch; every stride-th one is timed with events on stream s
   ProfScope(int cat, double flops, double bytes, cudaStream_t s);
   ~ProfScope();
@@ -175,6 +175,22 @@ int gemm_simt(int dtype, int layout, int M, int N, int K, const void* A, int lda
               const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s);
 int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
             void* C, int ldc, int out_f32_accum, cudaStream_t s, void* gelu_out = nullptr);
+// One GEMM as a value (same fields as gemm()'s arguments).
+struct GemmDesc {
+  int layout, M, N, K;
+  const void* A; int lda;
+  const void* B; int ldb;
+  const float* bias;
+  void* C; int ldc;
+  int out_f32_accum;
+  void* gelu_out;
+};
+int gemm_tc_multi(const GemmDesc* d, int n, cudaStream_t s);       // n <= 2 problems in ONE persistent launch
+// The backward pair of one linear layer y = x W^T: G_W += dy^T x (wgrad, beta = 1, Alg. 1 line 13) and dx = dy W
+// (dgrad with the CURRENT W, Eq. 1).  bf16: ONE tcgen05 launch whose CTA pairs share both problems' k-blocks evenly;
+// fp32: the two FFMA GEMMs.  dy [M, N_out] (row stride ld_dy), x [M, K_in], W [N_out, K_in], dx [M, K_in].
+int gemm_backward_pair(int dtype, int M, int N_out, int K_in, const void* dy, int ld_dy, const void* x, int ld_x,
+                       const void* W, int ld_w, float* G_W, int ld_g, void* dx, int ld_dx, cudaStream_t s);
 // C = A B^T + bias (pre-activation, stashed for backward) and Gout = gelu(C), both [M, N] with row stride ldc:
 // one launch on the tcgen05 path (GELU in the GEMM epilogue, rows a7 + a8), GEMM then gelu_fwd otherwise.
 int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,

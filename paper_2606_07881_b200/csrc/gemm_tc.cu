@@ -28,7 +28,11 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdlib>
+#include <cstring>
+#include <type_traits>
+#include <vector>
 #include <mutex>
 #include <unordered_map>
 
@@ -43,54 +47,105 @@ constexpr int BLOCK_M = 128;
 constexpr int BLOCK_K = 64;
 constexpr int UMMA_K = 16;
 constexpr int NUM_THREADS = 192;
-constexpr int EPI_BUFS = 3;                 // staging boxes per epilogue warp: a box is reused only after the TMA store
+constexpr int EPI_BUFS = 4;                 // staging boxes per epilogue warp: a box is reused only after the TMA store
                                             // issued EPI_BUFS chunks ago has read it (2 buffers left ~0.7 us of store
-                                            // latency exposed per chunk: 3.1 us of epilogue for the last tile of a launch)
+                                            // latency exposed per chunk); the GELU epilogue uses them as two PAIRS
 constexpr uint32_t EPI_STAGING_BYTES = 4 * EPI_BUFS * 4096;
+constexpr int MAX_WORKERS = 80;             // CTA pairs of one launch (74 on a B200)
+constexpr int MAX_PROB = 2;                 // problems per launch (a dgrad and the wgrad that shares its dy operand)
 
 using namespace tc;
 
-struct Params {
-  int M, N, K, ldc;
-  int tiles_m, tiles_n, splits, kb_total;
-  int range_mode;                                   // 1: workers own contiguous ranges of (tile, k-block) units
+// One GEMM of a launch.  Layout and epilogue are RUNTIME properties, so one kernel serves NT / NN / TN, the bf16 store
+// and the fp32 reduce-add epilogue, and two different problems can share one persistent grid.
+struct Prob {
+  int M, N, K;
+  int tiles_m, tiles_n, kb_total;
+  int splits;        // item mode: items = tile x split, dealt round-robin
+  int range_mode;    // 1: worker w owns the contiguous (tile, k-block) units [ustart[w], ustart[w+1])   (accum only)
+  int a_mn, b_mn;    // operand majors: 0 = K-major, 1 = MN-major
+  int accum;         // 0: C is bf16, overwritten, + bias;  1: C is fp32 and the product is ADDED (TMA reduce-add)
+  int gelu;          // !accum only: also store gelu(C) through the second map (MLP-up: rows a7 + a8)
   const float* bias;
-  void* C;
-  int gelu;       // !ACCUM only: also store gelu(C) through tmC2 (MLP-up: the pre-activation is stashed, rows a7 + a8)
+};
+struct Params {
+  Prob pr[MAX_PROB];
+  int n_prob;
+  int ustart[MAX_PROB][MAX_WORKERS + 1];
+};
+struct Maps { CUtensorMap a[MAX_PROB], b[MAX_PROB], c[MAX_PROB], c2; };
+
+// The work list of one CTA pair, walked identically by the producer, the MMA issuer and the epilogue warps: the
+// problems in order; inside a problem either whole items (tile x split, round-robin) or the worker's contiguous range
+// of (tile, k-block) units, cut wherever it crosses a tile boundary (partials meet in the L2 adders).
+struct Work {
+  int q, item;
+  long cur, end;
+  bool started;
+  __device__ __forceinline__ Work() : q(0), item(0), cur(0), end(0), started(false) {}
+  __device__ __forceinline__ bool next(const Params& p, int worker, int n_workers, int& tile, int& kb0, int& kb1) {
+    while (q < p.n_prob) {
+      const Prob& pr = p.pr[q];
+      if (!started) {
+        started = true;
+        if (pr.range_mode) { cur = p.ustart[q][worker]; end = p.ustart[q][worker + 1]; }
+        else item = worker;
+      }
+      if (pr.range_mode) {
+        if (cur < end) {
+          tile = (int)(cur / pr.kb_total);
+          kb0 = (int)(cur % pr.kb_total);
+          kb1 = (int)min((long)pr.kb_total, kb0 + (end - cur));
+          cur += kb1 - kb0;
+          return true;
+        }
+      } else {
+        const int kb_per = (pr.kb_total + pr.splits - 1) / pr.splits;
+        if (item < pr.tiles_m * pr.tiles_n * pr.splits) {
+          tile = item / pr.splits;
+          kb0 = (item % pr.splits) * kb_per;
+          kb1 = min(kb0 + kb_per, pr.kb_total);
+          item += n_workers;
+          return true;
+        }
+      }
+      ++q;
+      started = false;
+    }
+    return false;
+  }
 };
 
 // ------------------------------------------------------------------ the kernel
-// CG = 1: one CTA per tile of 128 x BLOCK_N.  CG = 2: a CTA pair (cluster of 2, same TPC) per tile of
-// 256 x BLOCK_N: CTA r owns rows m0 + 128 r .. of A and of the accumulator, and stages columns
-// n0 + r BLOCK_N/2 .. of B; the leader (rank 0) issues tcgen05.mma.cta_group::2 for both.
-template <int CG, int BLOCK_N, int STAGES, bool A_MN, bool B_MN, bool ACCUM>
+// A CTA pair (cluster of 2, same TPC) per tile of 256 x BLOCK_N: CTA r owns rows m0 + 128 r .. of A and of the
+// accumulator, and stages columns n0 + r BLOCK_N/2 .. of B; the leader (rank 0) issues tcgen05.mma.cta_group::2 for both.
+template <int BLOCK_N, int STAGES>
 __global__ void __launch_bounds__(NUM_THREADS, 1)
-gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB,
-               const __grid_constant__ CUtensorMap tmC, const __grid_constant__ CUtensorMap tmC2, const Params p) {
+gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params p) {
+  constexpr int CG = 2;
   constexpr int BN_CTA = BLOCK_N / CG;                  // B rows staged by one CTA
   constexpr uint32_t A_BYTES = BLOCK_M * BLOCK_K * 2, B_BYTES = BN_CTA * BLOCK_K * 2;
   constexpr uint32_t STAGE_BYTES = A_BYTES + B_BYTES;
   constexpr uint32_t BOX_MN_BYTES = 64 * BLOCK_K * 2;   // one {64 mn, 64 k} box of an MN-major operand
   constexpr uint32_t TMEM_COLS = 2 * BLOCK_N;
   // instruction descriptor: D fp32 (bit 4), A/B bf16 (bits 7, 10), majors (15, 16), N>>3 at 17, M>>4 at 24
-  constexpr uint32_t IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((A_MN ? 1u : 0u) << 15) |
-                             ((B_MN ? 1u : 0u) << 16) | ((uint32_t)(BLOCK_N >> 3) << 17) |
-                             ((uint32_t)((BLOCK_M * CG) >> 4) << 24);
+  constexpr uint32_t IDESC0 = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(BLOCK_N >> 3) << 17) |
+                              ((uint32_t)((BLOCK_M * CG) >> 4) << 24);
 
-  extern __shared__ __align__(1024) uint8_t smem_raw[];
-  uint8_t* smem = (uint8_t*)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint8_t* staging = smem + STAGES * STAGE_BYTES;        // 4 epilogue warps x EPI_BUFS buffers x 4 KB (1024-aligned)
-  float* bias_s = (float*)(staging + EPI_STAGING_BYTES); // 4 epilogue warps x BLOCK_N floats
-  uint64_t* full = (uint64_t*)(bias_s + 4 * BLOCK_N);
+  extern __shared__ __align__(1024) uint8_t smem[];     // 128B-swizzled tiles need 1024-byte alignment (checked below)
+  uint8_t* staging = smem + STAGES * STAGE_BYTES;        // 4 epilogue warps x EPI_BUFS buffers x 4 KB
+  float* bias_s = (float*)(staging + EPI_STAGING_BYTES); // 4 epilogue warps x 2 x 64 floats (chunk-wise, double-buffered)
+  uint64_t* full = (uint64_t*)(bias_s + 4 * 128);
   uint64_t* empty = full + STAGES;
   uint64_t* tfull = empty + STAGES;
   uint64_t* tempty = tfull + 2;
   uint32_t* tmem_slot = (uint32_t*)(tempty + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rank = CG == 2 ? cluster_ctarank() : 0u;
+  const uint32_t rank = cluster_ctarank();
   const bool leader = rank == 0;
 
+  if ((smem_u32(smem) & 1023u) != 0) __trap();
   if (threadIdx.x == 0) {
     for (int i = 0; i < STAGES; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 4 * CG); }
@@ -101,186 +156,189 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   // stream's multi-wave kernel shared the SMs (all other CTAs of the launch had finished; peer stuck in the second
   // barrier).  The second barrier makes both allocations (and both CTAs' mbarriers) exist before the leader's
   // first MMA writes the peer's TMEM.
-  if (CG == 2) { __syncthreads(); cluster_sync_all(); }
-  if (warp == 1) {
-    if (CG == 2) {
-      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
-                   "r"(TMEM_COLS) : "memory");
-    } else {
-      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
-                   "r"(TMEM_COLS) : "memory");
-      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-    }
-  }
+  __syncthreads();
+  cluster_sync_all();
+  if (warp == 1)
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)),
+                 "r"(TMEM_COLS) : "memory");
   tc_fence_before();
   __syncthreads();
-  if (CG == 2) {
-    cluster_sync_all();
-    if (warp == 1) asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
-  }
+  cluster_sync_all();
+  if (warp == 1) asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
 
-  const int n_items = p.tiles_m * p.tiles_n * p.splits;
-  const int kb_per = (p.kb_total + p.splits - 1) / p.splits;
-  const int worker = CG == 2 ? (int)(blockIdx.x >> 1) : (int)blockIdx.x;
-  const int n_workers = CG == 2 ? (int)(gridDim.x >> 1) : (int)gridDim.x;
-  // The work list of this CTA (pair), walked identically by the producer, the MMA issuer and the epilogue warps.
-  // Item mode: items = tile x split, dealt round-robin.  Range mode (fp32 reduce-add output only): the (tile,
-  // k-block) space is cut into n_workers equal contiguous ranges, so every worker does the same number of k-blocks
-  // and flushes its accumulator wherever its range crosses a tile boundary (partials meet in the L2 adders).
-  struct Work {
-    long cur, end;
-    int item, n_items, step, splits, kb_per, kb_total, range;
-    __device__ __forceinline__ bool next(int& tile, int& kb0, int& kb1) {
-      if (range) {
-        if (cur >= end) return false;
-        tile = (int)(cur / kb_total);
-        kb0 = (int)(cur % kb_total);
-        kb1 = (int)min((long)kb_total, kb0 + (end - cur));
-        cur += kb1 - kb0;
-        return true;
-      }
-      if (item >= n_items) return false;
-      tile = item / splits;
-      kb0 = (item % splits) * kb_per;
-      kb1 = min(kb0 + kb_per, kb_total);
-      item += step;
-      return true;
-    }
-  };
-  const long units = (long)p.tiles_m * p.tiles_n * p.kb_total;
-  const Work work0{units * worker / n_workers, units * (worker + 1) / n_workers, worker, n_items, n_workers, p.splits, kb_per,
-                   p.kb_total, p.range_mode};
+  const int worker = (int)(blockIdx.x >> 1);
+  const int n_workers = (int)(gridDim.x >> 1);
 
   if (warp == 0) {
     if (lane == 0) {
-      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmA) : "memory");
-      asm volatile("prefetch.tensormap [%0];" ::"l"(&tmB) : "memory");
+      for (int q = 0; q < p.n_prob; ++q) {
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a[q]) : "memory");
+        asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b[q]) : "memory");
+      }
       uint32_t stage = 0, phase = 0;
-      Work work = work0;
-      for (int tile, kb0, kb1; work.next(tile, kb0, kb1);) {
-        const int m0 = (tile % p.tiles_m) * (BLOCK_M * CG) + (int)rank * BLOCK_M;
-        const int n0 = (tile / p.tiles_m) * BLOCK_N + (int)rank * BN_CTA;
-        for (int kb = kb0; kb < kb1; ++kb) {
-          mbar_wait(&empty[stage], phase ^ 1, 1);
-          uint8_t* sa = smem + stage * STAGE_BYTES;
-          uint8_t* sb = sa + A_BYTES;
-          const int k0 = kb * BLOCK_K;
-          if (CG == 2) {
+      const uint32_t full0 = mapa_rank(smem_u32(&full[0]), 0);     // the LEADER's full[0]; full[i] is 8 i bytes further
+      const uint32_t smem0 = smem_u32(smem);
+      Work work;
+      for (int tile, kb0, kb1; work.next(p, worker, n_workers, tile, kb0, kb1);) {
+        const Prob& pr = p.pr[work.q];
+        const CUtensorMap* tmA = &maps.a[work.q];
+        const CUtensorMap* tmB = &maps.b[work.q];
+        const int m0 = (tile % pr.tiles_m) * (BLOCK_M * CG) + (int)rank * BLOCK_M;
+        const int n0 = (tile / pr.tiles_m) * BLOCK_N + (int)rank * BN_CTA;
+        // the k-block loop is specialised at compile time on the operand majors (a runtime layout flag inside it cost
+        // 7-11% of the GEMM: measured); the dispatch is per work item
+        auto kloop = [&](auto a_mn_t, auto b_mn_t) {
+          constexpr bool a_mn = decltype(a_mn_t)::value, b_mn = decltype(b_mn_t)::value;
+          for (int kb = kb0; kb < kb1; ++kb) {
+            mbar_wait_lean(&empty[stage], phase ^ 1);
+            const uint32_t sa = smem0 + stage * STAGE_BYTES, sb = sa + A_BYTES;
+            const int k0 = kb * BLOCK_K;
             // both CTAs' bytes are counted on the leader's barrier; its single arrival is this expect_tx
             if (leader) mbar_expect_tx(&full[stage], 2 * STAGE_BYTES);
-            const uint32_t bar = mapa_rank(smem_u32(&full[stage]), 0);
-            if (A_MN) {
+            const uint32_t bar = full0 + stage * 8;
+            if (a_mn) {
 #pragma unroll
-              for (int i = 0; i < BLOCK_M / 64; ++i) tma_load_2d_pair(sa + i * BOX_MN_BYTES, &tmA, bar, m0 + i * 64, k0);
+              for (int i = 0; i < BLOCK_M / 64; ++i) tma_load_2d_pair_s(sa + i * BOX_MN_BYTES, tmA, bar, m0 + i * 64, k0);
             } else {
-              tma_load_2d_pair(sa, &tmA, bar, k0, m0);
+              tma_load_2d_pair_s(sa, tmA, bar, k0, m0);
             }
-            if (B_MN) {
+            if (b_mn) {
 #pragma unroll
-              for (int i = 0; i < BN_CTA / 64; ++i) tma_load_2d_pair(sb + i * BOX_MN_BYTES, &tmB, bar, n0 + i * 64, k0);
+              for (int i = 0; i < BN_CTA / 64; ++i) tma_load_2d_pair_s(sb + i * BOX_MN_BYTES, tmB, bar, n0 + i * 64, k0);
             } else {
-              tma_load_2d_pair(sb, &tmB, bar, k0, n0);
+              tma_load_2d_pair_s(sb, tmB, bar, k0, n0);
             }
-          } else {
-            mbar_expect_tx(&full[stage], STAGE_BYTES);
-            if (A_MN) {
-#pragma unroll
-              for (int i = 0; i < BLOCK_M / 64; ++i) tma_load_2d(sa + i * BOX_MN_BYTES, &tmA, &full[stage], m0 + i * 64, k0);
-            } else {
-              tma_load_2d(sa, &tmA, &full[stage], k0, m0);
-            }
-            if (B_MN) {
-#pragma unroll
-              for (int i = 0; i < BN_CTA / 64; ++i) tma_load_2d(sb + i * BOX_MN_BYTES, &tmB, &full[stage], n0 + i * 64, k0);
-            } else {
-              tma_load_2d(sb, &tmB, &full[stage], k0, n0);
-            }
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
           }
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
-        }
+        };
+        if (!pr.b_mn) kloop(std::false_type{}, std::false_type{});          // NT
+        else if (!pr.a_mn) kloop(std::false_type{}, std::true_type{});      // NN
+        else kloop(std::true_type{}, std::true_type{});                     // TN
       }
     }
   } else if (warp == 1) {
     if (lane == 0 && leader) {
+      // The single issuing thread is on the critical path of every k-block (wait, fence, 4 MMAs, commit against 4 x 128
+      // tensor cycles), so everything that does not change per MMA is hoisted: a shared-memory descriptor is a constant
+      // per (problem, operand) plus the tile's address in 16-byte units, and a K = 16 step adds a constant to it.
       uint32_t stage = 0, phase = 0, acc = 0, acc_phase = 0;
-      Work work = work0;
-      for (int tile, kb0, kb1; work.next(tile, kb0, kb1);) {
-        mbar_wait(&tempty[acc], acc_phase ^ 1, 2);      // epilogue (of both CTAs) has drained this accumulator
+      const uint32_t smem16 = smem_u32(smem) >> 4;
+      Work work;
+      for (int tile, kb0, kb1; work.next(p, worker, n_workers, tile, kb0, kb1);) {
+        const Prob& pr = p.pr[work.q];
+        mbar_wait_lean(&tempty[acc], acc_phase ^ 1);    // epilogue (of both CTAs) has drained this accumulator
         tc_fence_after();
         const uint32_t tmem_d = tmem_base + acc * BLOCK_N;
-        for (int kb = kb0; kb < kb1; ++kb) {
-          mbar_wait(&full[stage], phase, 3);
-          tc_fence_after();
-          const uint32_t sa = smem_u32(smem + stage * STAGE_BYTES), sb = sa + A_BYTES;
+        auto kloop = [&](auto a_mn_t, auto b_mn_t) {
+          constexpr bool a_mn = decltype(a_mn_t)::value, b_mn = decltype(b_mn_t)::value;
+          constexpr uint32_t idesc = IDESC0 | ((a_mn ? 1u : 0u) << 15) | ((b_mn ? 1u : 0u) << 16);
+          constexpr uint32_t a_step = (a_mn ? UMMA_K * 128 : UMMA_K * 2) >> 4, b_step = (b_mn ? UMMA_K * 128 : UMMA_K * 2) >> 4;
+          const uint64_t adesc0 = a_mn ? smem_desc(0, BOX_MN_BYTES, 1024) : smem_desc(0, 16, 1024);
+          const uint64_t bdesc0 = b_mn ? smem_desc(0, BOX_MN_BYTES, 1024) : smem_desc(0, 16, 1024);
+          uint32_t accumulate = 0;
+          for (int kb = kb0; kb < kb1; ++kb) {
+            mbar_wait_lean(&full[stage], phase);
+            tc_fence_after();
+            const uint32_t sa16 = smem16 + stage * (STAGE_BYTES >> 4);
+            uint64_t ad = adesc0 + sa16, bd = bdesc0 + (sa16 + (A_BYTES >> 4));
 #pragma unroll
-          for (int j = 0; j < BLOCK_K / UMMA_K; ++j) {
-            const uint64_t ad = A_MN ? smem_desc(sa + j * (UMMA_K * 128), BOX_MN_BYTES, 1024)
-                                     : smem_desc(sa + j * (UMMA_K * 2), 16, 1024);
-            const uint64_t bd = B_MN ? smem_desc(sb + j * (UMMA_K * 128), BOX_MN_BYTES, 1024)
-                                     : smem_desc(sb + j * (UMMA_K * 2), 16, 1024);
-            if (CG == 2) umma_bf16_pair(tmem_d, ad, bd, IDESC, (kb > kb0 || j > 0) ? 1u : 0u);
-            else umma_bf16(tmem_d, ad, bd, IDESC, (kb > kb0 || j > 0) ? 1u : 0u);
+            for (int j = 0; j < BLOCK_K / UMMA_K; ++j) {
+              umma_bf16_pair(tmem_d, ad, bd, idesc, accumulate);
+              accumulate = 1;
+              ad += a_step;
+              bd += b_step;
+            }
+            umma_commit_pair(&empty[stage]);             // frees the stage
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
           }
-          if (CG == 2) umma_commit_pair(&empty[stage]); else umma_commit(&empty[stage]);   // frees the stage
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
-        }
-        if (CG == 2) umma_commit_pair(&tfull[acc]); else umma_commit(&tfull[acc]);         // -> epilogue
+        };
+        if (!pr.b_mn) kloop(std::false_type{}, std::false_type{});          // NT
+        else if (!pr.a_mn) kloop(std::false_type{}, std::true_type{});      // NN
+        else kloop(std::true_type{}, std::true_type{});                     // TN
+        umma_commit_pair(&tfull[acc]);                   // -> epilogue
         acc ^= 1;
         if (acc == 0) acc_phase ^= 1;
       }
     }
   } else {
     // ===== epilogue warps: TMEM -> registers -> swizzled smem -> TMA store / TMA reduce-add =====
-    // Warp w (TMEM lane quarter q = w & 3) owns 32 rows of the tile and a private pair of 4 KB staging
-    // buffers, so the four warps never synchronise with each other.  One TMA box = 32 rows x 128 bytes
-    // (64 bf16 or 32 fp32 columns), SWIZZLE_128B: 16-byte chunk c of row r sits at chunk c ^ (r & 7),
-    // which makes the row-per-thread st.shared.v4 conflict-free.  TMA clips the box at the tensor edge.
+    // Warp w (TMEM lane quarter q = w & 3) owns 32 rows of the tile and EPI_BUFS private 4 KB staging buffers, so the
+    // four warps never synchronise with each other.  One TMA box = 32 rows x 128 bytes (64 bf16 or 32 fp32 columns),
+    // SWIZZLE_128B: 16-byte chunk c of row r sits at chunk c ^ (r & 7), which makes the row-per-thread st.shared.v4
+    // conflict-free.  TMA clips the box at the tensor edge.
     const int q = warp & 3;
-    constexpr int CHUNK = ACCUM ? 32 : 64;            // columns per TMA box
     uint8_t* my_stage = staging + (warp - 2) * (EPI_BUFS * 4096);
-    float* my_bias = bias_s + (warp - 2) * BLOCK_N;
+    float* my_bias = bias_s + (warp - 2) * 128;
     uint32_t acc = 0, acc_phase = 0, sbuf = 0;
-    Work work = work0;
-    for (int tile, kb0, kb1; work.next(tile, kb0, kb1);) {
-      const int m0 = (tile % p.tiles_m) * (BLOCK_M * CG) + (int)rank * BLOCK_M, n0 = (tile / p.tiles_m) * BLOCK_N;
-      if (!ACCUM) {                                   // bias slice of this tile, fetched under the main loop
+    Work work;
+    for (int tile, kb0, kb1; work.next(p, worker, n_workers, tile, kb0, kb1);) {
+      const Prob& pr = p.pr[work.q];
+      const CUtensorMap* tmC = &maps.c[work.q];
+      const int m0 = (tile % pr.tiles_m) * (BLOCK_M * CG) + (int)rank * BLOCK_M, n0 = (tile / pr.tiles_m) * BLOCK_N;
+      const bool accum = pr.accum != 0;
+      // bias slice of this tile: lane l keeps columns l, l + 32, ... in registers (fetched under the main loop, so no
+      // global-load latency sits inside the chunk loop) and hands them to shared memory one 64-column chunk ahead
+      float breg[BLOCK_N / 32];
+      if (!accum) {
+        const float* bias = pr.bias;
+        const int N = pr.N;
 #pragma unroll
         for (int i = 0; i < BLOCK_N / 32; ++i) {
           const int col = n0 + i * 32 + lane;
-          my_bias[i * 32 + lane] = (p.bias != nullptr && col < p.N) ? __ldg(p.bias + col) : 0.f;
+          breg[i] = (bias != nullptr && col < N) ? __ldg(bias + col) : 0.f;
         }
+        my_bias[lane] = breg[0];
+        my_bias[32 + lane] = breg[1];
         __syncwarp();
       }
       mbar_wait_many(&tfull[acc], acc_phase, 4);     // 128 threads wait a whole main loop: sleep between polls
       tc_fence_after();
       const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + acc * BLOCK_N;
+      if (accum) {
 #pragma unroll 1
-      for (int c = 0; c < BLOCK_N; c += CHUNK) {
-        if (n0 + c >= p.N) break;                     // warp-uniform
-        const bool gelu = !ACCUM && p.gelu != 0;       // kernel-uniform
-        uint8_t* buf = gelu ? my_stage : my_stage + sbuf * 4096;
-        uint8_t* buf2 = my_stage + 4096;               // gelu: second output tile of the same chunk
-        if (!gelu) sbuf = sbuf + 1 == EPI_BUFS ? 0 : sbuf + 1;
-        if (lane == 0) { if (gelu) bulk_wait_read<0>(); else bulk_wait_read<EPI_BUFS - 1>(); }   // staging buffer(s) free again
-        __syncwarp();
-        uint8_t* rowp = buf + lane * 128;
-        if (ACCUM) {
+        for (int c = 0; c < BLOCK_N; c += 32) {
+          if (n0 + c >= pr.N) break;                  // warp-uniform
+          uint8_t* buf = my_stage + sbuf * 4096;
+          sbuf = (sbuf + 1) % EPI_BUFS;
+          if (lane == 0) bulk_wait_read<EPI_BUFS - 1>();   // this staging buffer is free again
+          __syncwarp();
+          uint8_t* rowp = buf + lane * 128;
           uint32_t r[32];
           tmem_ld32(taddr + c, r);
 #pragma unroll
           for (int i = 0; i < 8; ++i)
             sts128(rowp + ((i ^ (lane & 7)) << 4), r[4 * i], r[4 * i + 1], r[4 * i + 2], r[4 * i + 3]);
-        } else {
+          fence_async_smem();                         // generic-proxy writes -> visible to the TMA engine
+          __syncwarp();
+          if (lane == 0) {
+            tma_reduce_add_2d(tmC, buf, n0 + c, m0 + q * 32);
+            bulk_commit();
+          }
+        }
+      } else {
+        const bool gelu = pr.gelu != 0;                // launch-uniform
+        int half = 0;
+#pragma unroll 1
+        for (int c = 0; c < BLOCK_N; c += 64, half ^= 1) {
+          if (n0 + c >= pr.N) break;                  // warp-uniform
+          // staging: one buffer per chunk, or (GELU) a pair: pre-activation and activation tile of the same chunk
+          uint8_t* buf = my_stage + sbuf * 4096;
+          uint8_t* buf2 = buf + 4096;
+          sbuf = (sbuf + (gelu ? 2 : 1)) % EPI_BUFS;
+          if (lane == 0) { if (gelu) bulk_wait_read<EPI_BUFS / 2 - 1>(); else bulk_wait_read<EPI_BUFS - 1>(); }
+          __syncwarp();
+          uint8_t* rowp = buf + lane * 128;
           uint32_t r64[64];                            // both halves of the chunk in flight before one wait
           tmem_ld32_nowait(taddr + c, r64);
           tmem_ld32_nowait(taddr + c + 32, r64 + 32);
           // the chunk's 64 bias values go to registers up front: interleaved with the (volatile, memory-
           // clobbering) st.shared they serialised into 8 load -> add -> store chains, 0.4 us per chunk
           float4 bq[16];
+          const float* bsrc = my_bias + half * 64;
 #pragma unroll
-          for (int k = 0; k < 16; ++k) bq[k] = *reinterpret_cast<const float4*>(my_bias + c + 4 * k);
+          for (int k = 0; k < 16; ++k) bq[k] = *reinterpret_cast<const float4*>(bsrc + 4 * k);
           tmem_ld_wait();
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
@@ -305,22 +363,27 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
               }
             }
           }
-        }
-        fence_async_smem();                           // generic-proxy writes -> visible to the TMA engine
-        __syncwarp();
-        if (lane == 0) {
-          if (ACCUM) tma_reduce_add_2d(&tmC, buf, n0 + c, m0 + q * 32);
-          else tma_store_2d(&tmC, buf, n0 + c, m0 + q * 32);
-          if (gelu) tma_store_2d(&tmC2, buf2, n0 + c, m0 + q * 32);
-          bulk_commit();
+          if (c + 64 < BLOCK_N) {                      // next chunk's bias -> the other half (c is warp-uniform)
+            const int i2 = (c >> 5) + 2;
+            float nb0 = 0.f, nb1 = 0.f;
+#pragma unroll
+            for (int i = 2; i < BLOCK_N / 32; i += 2)
+              if (i == i2) { nb0 = breg[i]; nb1 = breg[i + 1]; }
+            my_bias[(half ^ 1) * 64 + lane] = nb0;
+            my_bias[(half ^ 1) * 64 + 32 + lane] = nb1;
+          }
+          fence_async_smem();                         // generic-proxy writes -> visible to the TMA engine
+          __syncwarp();
+          if (lane == 0) {
+            tma_store_2d(tmC, buf, n0 + c, m0 + q * 32);
+            if (gelu) tma_store_2d(&maps.c2, buf2, n0 + c, m0 + q * 32);
+            bulk_commit();
+          }
         }
       }
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) {
-        if (CG == 2) mbar_arrive_cluster(mapa_rank(smem_u32(&tempty[acc]), 0));
-        else mbar_arrive(&tempty[acc]);
-      }
+      if (lane == 0) mbar_arrive_cluster(mapa_rank(smem_u32(&tempty[acc]), 0));
       acc ^= 1;
       if (acc == 0) acc_phase ^= 1;
     }
@@ -329,15 +392,12 @@ gemm_tc_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ 
   }
   tc_fence_before();
   __syncthreads();
-  if (CG == 2) cluster_sync_all();                     // no CTA leaves while its pair can still signal it
+  cluster_sync_all();                                  // no CTA leaves while its pair can still signal it
   if (warp == 1) {
     tc_fence_after();
-    if (CG == 2)
-      asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
-    else
-      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(TMEM_COLS) : "memory");
   }
-  if (CG == 2) cluster_sync_all();                     // pair-wide dealloc: neither CTA exits before both freed
+  cluster_sync_all();                                  // pair-wide dealloc: neither CTA exits before both freed
 }
 
 // ------------------------------------------------------------------ host: tensor maps
@@ -402,13 +462,12 @@ int make_map(CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1, uint64
 }
 
 
-template <int CG, int BLOCK_N, int STAGES, bool A_MN, bool B_MN, bool ACCUM>
-int launch(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tmC, const CUtensorMap& tmC2,
-           const Params& p, int grid, cudaStream_t s) {
-  constexpr size_t SMEM = (size_t)STAGES * (BLOCK_M * BLOCK_K * 2 + (BLOCK_N / CG) * BLOCK_K * 2) +
-                          EPI_STAGING_BYTES + 4 * BLOCK_N * 4 + 1024 + 256;
+template <int BLOCK_N, int STAGES>
+int launch(const Maps& maps, const Params& p, int grid, cudaStream_t s) {
+  constexpr size_t SMEM = (size_t)STAGES * (BLOCK_M * BLOCK_K * 2 + (BLOCK_N / 2) * BLOCK_K * 2) + EPI_STAGING_BYTES +
+                          4 * 128 * 4 + 256;
   static_assert(SMEM <= 232448, "shared memory budget of one sm_100 CTA");
-  auto kern = gemm_tc_kernel<CG, BLOCK_N, STAGES, A_MN, B_MN, ACCUM>;
+  auto kern = gemm_tc_kernel<BLOCK_N, STAGES>;
   { int rc_ = set_max_dynamic_smem((const void*)kern, (int)SMEM); if (rc_) return rc_; }
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(grid);
@@ -417,17 +476,48 @@ int launch(const CUtensorMap& tmA, const CUtensorMap& tmB, const CUtensorMap& tm
   cfg.stream = s;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = CG;
+  attr[0].val.clusterDim.x = 2;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  PACI_CUDA_OK(cudaLaunchKernelEx(&cfg, kern, tmA, tmB, tmC, tmC2, p));
+  PACI_CUDA_OK(cudaLaunchKernelEx(&cfg, kern, maps, p));
   g_launches.fetch_add(1, std::memory_order_relaxed);
   return PACI_OK;
 }
 
 thread_local int32_t g_last_plan[6] = {0, 0, 0, 0, 0, 0};
+
+// validates one problem and fills its Prob + tensor maps
+int fill_problem(const GemmDesc& d, int BN, Prob* pr, CUtensorMap* tmA, CUtensorMap* tmB, CUtensorMap* tmC,
+                 CUtensorMap* tmC2) {
+  if (d.gelu_out != nullptr && (d.out_f32_accum || (uintptr_t)d.gelu_out % 16))
+    return fail(PACI_EINVAL, "tcgen05 GEMM: gelu output needs the bf16 epilogue and a 16-byte aligned pointer");
+  if (d.K <= 0) return fail(PACI_EINVAL, "tcgen05 GEMM: K=%d", d.K);
+  if (d.layout < 0 || d.layout > 2) return fail(PACI_EINVAL, "gemm: layout %d", d.layout);
+  if ((uintptr_t)d.C % 16 || (d.out_f32_accum ? d.ldc % 4 : d.ldc % 8))
+    return fail(PACI_EINVAL, "tcgen05 GEMM: C not 16-byte aligned (ldc=%d)", d.ldc);
+  if (d.bias != nullptr && (uintptr_t)d.bias % 16) return fail(PACI_EINVAL, "tcgen05 GEMM: bias not 16-byte aligned");
+  const bool a_mn = d.layout == 2, b_mn = d.layout != 0;
+  int rc;
+  // A: K-major [M rows][K contiguous] -> dims {K, M}, box {64, 128};  MN-major [K rows][M contiguous] -> {M, K}, {64, 64}
+  rc = a_mn ? make_map(tmA, d.A, d.M, d.K, d.lda, 64, BLOCK_K) : make_map(tmA, d.A, d.K, d.M, d.lda, BLOCK_K, BLOCK_M);
+  if (rc) return rc;
+  rc = b_mn ? make_map(tmB, d.B, d.N, d.K, d.ldb, 64, BLOCK_K) : make_map(tmB, d.B, d.K, d.N, d.ldb, BLOCK_K, BN / 2);
+  if (rc) return rc;
+  // C: box of 32 rows x 128 bytes, written by one epilogue warp per TMA store / reduce-add
+  rc = d.out_f32_accum ? make_map(tmC, d.C, d.N, d.M, d.ldc, 32, 32, 4) : make_map(tmC, d.C, d.N, d.M, d.ldc, 64, 32, 2);
+  if (rc) return rc;
+  if (d.gelu_out != nullptr && (rc = make_map(tmC2, d.gelu_out, d.N, d.M, d.ldc, 64, 32, 2))) return rc;
+  pr->M = d.M; pr->N = d.N; pr->K = d.K;
+  pr->tiles_m = ceil_div(d.M, BLOCK_M * 2);
+  pr->tiles_n = ceil_div(d.N, BN);
+  pr->kb_total = ceil_div(d.K, BLOCK_K);
+  pr->splits = 1; pr->range_mode = 0;
+  pr->a_mn = a_mn; pr->b_mn = b_mn; pr->accum = d.out_f32_accum != 0; pr->gelu = d.gelu_out != nullptr;
+  pr->bias = d.bias;
+  return PACI_OK;
+}
 
 }  // namespace
 
@@ -436,91 +526,127 @@ int make_tensor_map(CUtensorMap* out, const void* ptr, uint64_t d0, uint64_t d1,
   return make_map(out, ptr, d0, d1, ld, b0, b1, esz);
 }
 
-int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
-            void* C, int ldc, int out_f32_accum, cudaStream_t s, void* gelu_out) {
-  if (M <= 0 || N <= 0) return PACI_OK;
-  if (gelu_out != nullptr && (out_f32_accum || (uintptr_t)gelu_out % 16))
-    return fail(PACI_EINVAL, "tcgen05 GEMM: gelu output needs the bf16 epilogue and a 16-byte aligned pointer");
-  if (K <= 0) return fail(PACI_EINVAL, "tcgen05 GEMM: K=%d", K);
-  if (layout < 0 || layout > 2) return fail(PACI_EINVAL, "gemm: layout %d", layout);
-  if ((uintptr_t)C % 16 || (out_f32_accum ? ldc % 4 : ldc % 8))
-    return fail(PACI_EINVAL, "tcgen05 GEMM: C not 16-byte aligned (ldc=%d)", ldc);
-  if (bias != nullptr && (uintptr_t)bias % 16) return fail(PACI_EINVAL, "tcgen05 GEMM: bias not 16-byte aligned");
-  const bool a_mn = layout == 2, b_mn = layout != 0;
-  constexpr int CG = 2;                              // CTA pair (cluster of 2, one TPC) per 256-row tile
-  const int BN = N <= 128 ? 128 : 256;
-  CUtensorMap tmA, tmB, tmC, tmC2;
-  int rc;
-  // A: K-major [M rows][K contiguous] -> dims {K, M}, box {64, 128};  MN-major [K rows][M contiguous] -> {M, K}, {64, 64}
-  rc = a_mn ? make_map(&tmA, A, M, K, lda, 64, BLOCK_K) : make_map(&tmA, A, K, M, lda, BLOCK_K, BLOCK_M);
-  if (rc) return rc;
-  rc = b_mn ? make_map(&tmB, B, N, K, ldb, 64, BLOCK_K) : make_map(&tmB, B, K, N, ldb, BLOCK_K, BN / CG);
-  if (rc) return rc;
-  // C: box of 32 rows x 128 bytes, written by one epilogue warp per TMA store / reduce-add
-  rc = out_f32_accum ? make_map(&tmC, C, N, M, ldc, 32, 32, 4) : make_map(&tmC, C, N, M, ldc, 64, 32, 2);
-  if (rc) return rc;
-  tmC2 = tmC;
-  if (gelu_out != nullptr && (rc = make_map(&tmC2, gelu_out, N, M, ldc, 64, 32, 2))) return rc;
-  Params p;
-  p.M = M; p.N = N; p.K = K; p.ldc = ldc; p.bias = bias; p.C = C; p.gelu = gelu_out != nullptr;
-  p.tiles_m = ceil_div(M, BLOCK_M * CG);
-  p.tiles_n = ceil_div(N, BN);
-  p.kb_total = ceil_div(K, BLOCK_K);
-  const int tiles = p.tiles_m * p.tiles_n, workers = std::max(1, num_sms() / CG);
-  int splits = 1;
-  if (out_f32_accum) {
-    // split-K over the contraction (tokens): partials meet in the fp32 TMA reduce-add epilogue.  Cost model in
-    // k-block units: rounds of the persistent grid x (k-blocks per item + EPI), where EPI ~ 8 k-blocks stands
-    // for an item's reduce-add epilogue (every extra split re-sends the whole fp32 tile through the L2 adders:
-    // 8 splits of the 4096x1024 wgrad measured 73 us against 1 split's 1.73-round quantisation loss).
-    const int max_s = std::max(1, std::min(p.kb_total / 4, 32));
-    const int EPI = 8;
-    long best = -1;
-    for (int sp = 1; sp <= max_s; ++sp) {
-      const int kb_per = ceil_div(p.kb_total, sp);
-      if (ceil_div(p.kb_total, kb_per) != sp) continue;        // every split owns at least one k-block
-      const long rounds = ceil_div((long)tiles * sp, workers);
-      const long cost = rounds * (kb_per + EPI);
-      if (best < 0 || cost < best) { best = cost; splits = sp; }
+// One launch for n <= 2 problems.  n == 2 is the backward pair of one linear layer: the wgrad (fp32 reduce-add output:
+// arbitrarily divisible along its contraction) and the dgrad (bf16 output: whole tiles).  The dgrad's tiles are dealt
+// round-robin over the CTA pairs, then the wgrad's (tile, k-block) units are poured on top until every pair carries
+// the same number of k-blocks ("water-filling"), so the pair of GEMMs has ONE prologue, ONE pipeline fill, ONE exposed
+// epilogue and no round quantisation (the 8192 x 1024 x 1024 dgrad alone: 128 tiles on 74 pairs = 1.73 rounds).
+int gemm_tc_multi(const GemmDesc* d, int n, cudaStream_t s) {
+  if (n < 1 || n > MAX_PROB) return fail(PACI_EINVAL, "gemm_tc_multi: n=%d", n);
+  for (int i = 0; i < n; ++i)
+    if (d[i].M <= 0 || d[i].N <= 0) {                  // an empty problem: launch the rest
+      if (n == 1) return PACI_OK;
+      return gemm_tc_multi(d + (i == 0 ? 1 : 0), 1, s);
+    }
+  if (n == 2) {
+    const bool small0 = d[0].N <= 128, small1 = d[1].N <= 128;
+    // the shared grid needs one tile width, the fp32 output first and no GELU output
+    if (small0 != small1 || !d[0].out_f32_accum || d[1].out_f32_accum || d[0].gelu_out || d[1].gelu_out) {
+      int rc = gemm_tc_multi(d, 1, s);
+      return rc ? rc : gemm_tc_multi(d + 1, 1, s);
     }
   }
-  p.splits = splits;
-  p.range_mode = 0;
-  if (out_f32_accum) {
-    // equal contiguous (tile, k-block) ranges instead of whole items: U / W k-blocks per worker plus one flush per
-    // tile boundary crossed (+1).  Taken for outputs of many rounds (the LM-head wgrad: 788 tiles, 10.65 rounds ->
-    // 0.659 to 0.597 ms); with fewer tiles than two rounds the k-block rate itself drops when every pair is busy
-    // and the round-robin splits measured the same or better
-    const int EPI = 8;
-    const long units = (long)tiles * p.kb_total;
-    const long per = ceil_div(units, (long)workers);
-    const long cost = per + (ceil_div(per, (long)p.kb_total) + 1) * EPI;
-    const long item_cost = ceil_div((long)tiles * splits, (long)workers) * (ceil_div(p.kb_total, splits) + EPI);
-    if (tiles >= 2 * workers && cost < item_cost) p.range_mode = 1;
+  const int BN = d[0].N <= 128 ? 128 : 256;
+  Maps maps;
+  Params p;
+  std::memset(&p, 0, sizeof p);
+  p.n_prob = n;
+  for (int i = 0; i < n; ++i) {
+    maps.c2 = maps.c[0];
+    int rc = fill_problem(d[i], BN, &p.pr[i], &maps.a[i], &maps.b[i], &maps.c[i], &maps.c2);
+    if (rc) return rc;
   }
-  // balanced persistent grid: the same number of rounds on the fewest workers (128 tiles on 74 pairs take 2
-  // rounds; so do 64 pairs, and the other 20 SMs stay free for the other stage streams' kernels)
-  const int items = tiles * splits;
-  const int rounds = ceil_div(items, workers);
-  const int grid = (p.range_mode ? workers : ceil_div(items, rounds)) * CG;
-#define GO(CG_, BN_, ST_, AMN, BMN, ACC) return launch<CG_, BN_, ST_, AMN, BMN, ACC>(tmA, tmB, tmC, tmC2, p, grid, s)
-#define BY_LAYOUT(CG_, BN_, ST_)                                                                          \
-  do {                                                                                                    \
-    if (out_f32_accum) {                                                                                  \
-      if (layout == 0) GO(CG_, BN_, ST_, false, false, true);                                             \
-      if (layout == 1) GO(CG_, BN_, ST_, false, true, true);                                              \
-      GO(CG_, BN_, ST_, true, true, true);                                                                \
-    }                                                                                                     \
-    if (layout == 0) GO(CG_, BN_, ST_, false, false, false);                                              \
-    if (layout == 1) GO(CG_, BN_, ST_, false, true, false);                                               \
-    GO(CG_, BN_, ST_, true, true, false);                                                                 \
-  } while (0)
-  g_last_plan[0] = CG; g_last_plan[1] = BN; g_last_plan[2] = splits; g_last_plan[3] = p.range_mode;
-  g_last_plan[4] = grid; g_last_plan[5] = tiles;
-  if (BN == 128) BY_LAYOUT(2, 128, 7);
-  BY_LAYOUT(2, 256, 5);
-#undef BY_LAYOUT
-#undef GO
+  if (n == 1) { maps.a[1] = maps.a[0]; maps.b[1] = maps.b[0]; maps.c[1] = maps.c[0]; if (!d[0].gelu_out) maps.c2 = maps.c[0]; }
+  const int workers = std::min(std::max(1, num_sms() / 2), MAX_WORKERS);
+  int grid;
+  if (n == 1) {
+    Prob& pr = p.pr[0];
+    const int tiles = pr.tiles_m * pr.tiles_n;
+    int splits = 1;
+    if (pr.accum) {
+      // split-K over the contraction (tokens): partials meet in the fp32 TMA reduce-add epilogue.  Cost model in
+      // k-block units: rounds of the persistent grid x (k-blocks per item + EPI), where EPI ~ 8 k-blocks stands
+      // for an item's reduce-add epilogue (every extra split re-sends the whole fp32 tile through the L2 adders:
+      // 8 splits of the 4096x1024 wgrad measured 73 us against 1 split's 1.73-round quantisation loss).
+      const int max_s = std::max(1, std::min(pr.kb_total / 4, 32));
+      const int EPI = 8;
+      long best = -1;
+      for (int sp = 1; sp <= max_s; ++sp) {
+        const int kb_per = ceil_div(pr.kb_total, sp);
+        if (ceil_div(pr.kb_total, kb_per) != sp) continue;        // every split owns at least one k-block
+        const long rounds = ceil_div((long)tiles * sp, workers);
+        const long cost = rounds * (kb_per + EPI);
+        if (best < 0 || cost < best) { best = cost; splits = sp; }
+      }
+      // equal contiguous (tile, k-block) ranges instead of whole items: U / W k-blocks per worker plus one flush per
+      // tile boundary crossed (+1).  Taken for outputs of many rounds (the LM-head wgrad: 788 tiles, 10.65 rounds ->
+      // 0.659 to 0.597 ms); with fewer tiles than two rounds the k-block rate itself drops when every pair is busy
+      // and the round-robin splits measured the same or better
+      const long units = (long)tiles * pr.kb_total;
+      const long per = ceil_div(units, (long)workers);
+      const long cost = per + (ceil_div(per, (long)pr.kb_total) + 1) * EPI;
+      const long item_cost = ceil_div((long)tiles * splits, (long)workers) * (ceil_div(pr.kb_total, splits) + EPI);
+      if (tiles >= 2 * workers && cost < item_cost) {
+        pr.range_mode = 1;
+        for (int w = 0; w <= workers; ++w) p.ustart[0][w] = (int)(units * w / workers);
+      }
+    }
+    pr.splits = splits;
+    // balanced persistent grid: the same number of rounds on the fewest workers (128 tiles on 74 pairs take 2
+    // rounds; so do 64 pairs, and the other 20 SMs stay free for the other stage streams' kernels)
+    const int items = tiles * splits;
+    const int rounds = ceil_div(items, workers);
+    grid = (pr.range_mode ? workers : ceil_div(items, rounds)) * 2;
+    g_last_plan[0] = 2; g_last_plan[1] = BN; g_last_plan[2] = splits; g_last_plan[3] = pr.range_mode;
+    g_last_plan[4] = grid; g_last_plan[5] = tiles;
+  } else {
+    // problem 0 = wgrad (range mode, poured second), problem 1 = dgrad (whole tiles, round-robin).  The kernel walks
+    // the wgrad range FIRST so that the launch's last, exposed epilogue is the cheaper bf16 store.
+    Prob& wg = p.pr[0];
+    Prob& dg = p.pr[1];
+    const int tiles_d = dg.tiles_m * dg.tiles_n;
+    const long U = (long)wg.tiles_m * wg.tiles_n * wg.kb_total;
+    std::vector<long> load(workers);
+    long total = U;
+    for (int w = 0; w < workers; ++w) {
+      load[w] = (long)((tiles_d - w + workers - 1) / workers) * dg.kb_total;   // tiles w, w + W, ...
+      if (tiles_d <= w) load[w] = 0;
+      total += load[w];
+    }
+    // water level T: sum_w max(0, T - load[w]) = U
+    std::vector<long> sorted(load);
+    std::sort(sorted.begin(), sorted.end());
+    double level = 0.0;
+    {
+      long acc = 0;
+      for (int i = 0; i < workers; ++i) {               // the i + 1 lightest workers fill up to `level`
+        acc += sorted[i];
+        level = (double)(U + acc) / (double)(i + 1);
+        if (i + 1 == workers || level <= (double)sorted[i + 1]) break;
+      }
+    }
+    double cum = 0.0;
+    p.ustart[0][0] = 0;
+    for (int w = 0; w < workers; ++w) {
+      cum += std::max(0.0, level - (double)load[w]);
+      p.ustart[0][w + 1] = (int)std::min<long>(U, (long)std::llround(cum));
+    }
+    p.ustart[0][workers] = (int)U;
+    wg.range_mode = 1;
+    dg.range_mode = 0; dg.splits = 1;
+    grid = workers * 2;
+    g_last_plan[0] = 2; g_last_plan[1] = BN; g_last_plan[2] = 2; g_last_plan[3] = 2;
+    g_last_plan[4] = grid; g_last_plan[5] = tiles_d + wg.tiles_m * wg.tiles_n;
+    (void)total;
+  }
+  if (BN == 128) return launch<128, 6>(maps, p, grid, s);
+  return launch<256, 5>(maps, p, grid, s);
+}
+
+int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
+            void* C, int ldc, int out_f32_accum, cudaStream_t s, void* gelu_out) {
+  GemmDesc d{layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, gelu_out};
+  return gemm_tc_multi(&d, 1, s);
 }
 
 void gemm_tc_last_plan(int32_t* out6) {

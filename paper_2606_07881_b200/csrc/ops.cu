@@ -19,6 +19,21 @@ int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, con
   return gemm_simt(dtype, layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, s);
 }
 
+int gemm_backward_pair(int dtype, int M, int N_out, int K_in, const void* dy, int ld_dy, const void* x, int ld_x,
+                       const void* W, int ld_w, float* G_W, int ld_g, void* dx, int ld_dx, cudaStream_t s) {
+  if (dtype == PACI_BF16) {
+    ProfScope prof(PC_GEMM_BWD_PAIR, 4.0 * M * (double)N_out * K_in,
+                   2.0 * (2.0 * (double)M * N_out + (double)M * K_in + (double)N_out * K_in) + 8.0 * N_out * K_in + 2.0 * M * K_in, s);
+    const GemmDesc d[2] = {
+        {2, N_out, K_in, M, dy, ld_dy, x, ld_x, nullptr, G_W, ld_g, 1, nullptr},      // G_W += dy^T x
+        {1, M, K_in, N_out, dy, ld_dy, W, ld_w, nullptr, dx, ld_dx, 0, nullptr}};     // dx = dy W
+    return gemm_tc_multi(d, 2, s);
+  }
+  int rc = gemm(dtype, 1, M, K_in, N_out, dy, ld_dy, W, ld_w, nullptr, dx, ld_dx, 0, s);
+  if (rc != PACI_OK) return rc;
+  return gemm(dtype, 2, N_out, K_in, M, dy, ld_dy, x, ld_x, nullptr, G_W, ld_g, 1, s);
+}
+
 int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
                    void* C, void* Gout, int ldc, cudaStream_t s) {
   if (dtype == PACI_BF16) {
@@ -80,6 +95,10 @@ extern "C" {
 int paci_op_gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
                  const float* bias, void* C, int ldc, int out_f32_accum, void* stream) {
   return gemm(dtype, layout, M, N, K, A, lda, B, ldb, bias, C, ldc, out_f32_accum, (cudaStream_t)stream);
+}
+int paci_op_gemm_backward_pair(int dtype, int M, int N_out, int K_in, const void* dy, int ld_dy, const void* x, int ld_x,
+                               const void* W, int ld_w, float* G_W, int ld_g, void* dx, int ld_dx, void* stream) {
+  return gemm_backward_pair(dtype, M, N_out, K_in, dy, ld_dy, x, ld_x, W, ld_w, G_W, ld_g, dx, ld_dx, (cudaStream_t)stream);
 }
 int paci_op_gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
                            const float* bias, void* C, void* G, int ldc, void* stream) {

@@ -38,7 +38,7 @@ cudaEvent_t take_event() {
 }
 const char* const kNames[PACI_PROF_NCAT] = {
     "gemm_fwd", "gemm_dgrad", "gemm_wgrad", "attention_fwd", "attention_bwd", "layernorm_fwd", "layernorm_bwd",
-    "gelu_fwd", "gelu_bwd", "colsum", "embedding", "softmax_ce", "adamw", "other"};
+    "gelu_fwd", "gelu_bwd", "colsum", "embedding", "softmax_ce", "adamw", "other", "gemm_bwd_pair"};
 }  // namespace
 
 ProfScope::ProfScope(int cat, double flops, double bytes, cudaStream_t s) : idx_(-1), stream_(s) {

@@ -470,14 +470,12 @@ static int backward_impl(paci_stage* st, char* act, const int32_t* tok, const vo
       RC(colsum(dt, M, D, dcur, pending_b2, cs));
       pending_b2 = nullptr;
     }
-    // MLP-down: dg = dm W2 ; G_W2 += dm^T g
-    RC(gemm(dt, 1, M, 4 * D, D, dm, D, w.w2.wc, 4 * D, nullptr, st->sc_d4, 4 * D, 0, cs));
-    RC(gemm(dt, 2, D, 4 * D, M, dm, D, act + b.g, 4 * D, nullptr, w.w2.g, 4 * D, 1, cs));
+    // MLP-down: dg = dm W2 ; G_W2 += dm^T g   (a13 + a14: one launch for the pair)
+    RC(gemm_backward_pair(dt, M, D, 4 * D, dm, D, act + b.g, 4 * D, w.w2.wc, 4 * D, w.w2.g, 4 * D, st->sc_d4, 4 * D, cs));
     // a16: dp = dg * gelu'(p) in place ; G_b1 += colsum(dp)
     RC(gelu_bwd(dt, M, 4 * D, st->sc_d4, act + b.p, st->sc_d4, w.b1.g, cs));
     // MLP-up: dy2 = dp W1 ; G_W1 += dp^T y2
-    RC(gemm(dt, 1, M, D, 4 * D, st->sc_d4, 4 * D, w.w1.wc, D, nullptr, st->sc_dD, D, 0, cs));
-    RC(gemm(dt, 2, 4 * D, D, M, st->sc_d4, 4 * D, act + b.y2, D, nullptr, w.w1.g, D, 1, cs));
+    RC(gemm_backward_pair(dt, M, 4 * D, D, st->sc_d4, 4 * D, act + b.y2, D, w.w1.wc, D, w.w1.g, D, st->sc_dD, D, cs));
     // a18: dx1 = dcur + LN2bwd(dy2) ; G_ln2 ; G_bo += colsum(dx1) (no dropout)
     RC(ln_bwd(dt, M, D, st->sc_dD, act + b.x1, (float*)(act + b.mean2), (float*)(act + b.rstd2), w.ln2g.w, dcur,
               st->sc_dx1, w.ln2g.g, w.ln2b.g, drop ? nullptr : w.bo.g, cs));
@@ -488,14 +486,12 @@ static int backward_impl(paci_stage* st, char* act, const int32_t* tok, const vo
       da = st->sc_dmask;
     }
     // out-proj: do = da Wo ; G_Wo += da^T o
-    RC(gemm(dt, 1, M, D, D, da, D, w.wo.wc, D, nullptr, st->sc_dD2, D, 0, cs));
-    RC(gemm(dt, 2, D, D, M, da, D, act + b.o, D, nullptr, w.wo.g, D, 1, cs));
+    RC(gemm_backward_pair(dt, M, D, D, da, D, act + b.o, D, w.wo.wc, D, w.wo.g, D, st->sc_dD2, D, cs));
     // a17: attention backward
     RC(attention_bwd(dt, n_seq, st->T, st->H, st->dh, st->sc_dD2, act + b.qkv, act + b.o,
                      (float*)(act + b.lse), st->sc_dqkv, st->sc_attn, w.bqkv.g, cs));   // + G_bqkv (a15)
     // QKV: dy1 = dqkv Wqkv ; G_Wqkv += dqkv^T y1
-    RC(gemm(dt, 1, M, D, 3 * D, st->sc_dqkv, 3 * D, w.wqkv.wc, D, nullptr, st->sc_dD, D, 0, cs));
-    RC(gemm(dt, 2, 3 * D, D, M, st->sc_dqkv, 3 * D, act + b.y1, D, nullptr, w.wqkv.g, D, 1, cs));
+    RC(gemm_backward_pair(dt, M, 3 * D, D, st->sc_dqkv, 3 * D, act + b.y1, D, w.wqkv.wc, D, w.wqkv.g, D, st->sc_dD, D, cs));
     // a18: dx = dx1 + LN1bwd(dy1) ; G_ln1 ; colsum(dx) is the previous block's G_b2 (no dropout)
     float* gcol = (!drop && l > 0) ? st->bw[l - 1].b2.g : nullptr;
     void* dst = (l == 0 && !st->cfg.has_embedding) ? din : (void*)pp[flip];

@@ -175,3 +175,30 @@ def test_single_stage_tied_head_bf16_full_vocab():
     """configs[4]'s structure: ONE stage holding the embedding, a block and the TIED head (R10: one tensor, the
     gradient of wte is the head wgrad PLUS the embedding scatter-add) at D = 1280, H = 20, V = 50257, T = 1024."""
     _stage_vs_oracle(1280, 20, 0, 1, 1)
+
+
+@pytest.mark.parametrize("M,N_out,K_in", [(8192, 1024, 1024), (8192, 1024, 4096), (8192, 4096, 1024), (8192, 3072, 1024),
+                                          (16384, 1280, 5120), (8192, 2304, 768)])
+def test_backward_pair_full_size_sampled(M, N_out, K_in):
+    """The one-launch dgrad + wgrad pair at the block shapes of configs[2] (and one each of configs[4], configs[1]):
+    sampled rows of dx and of G_W (pre-filled, beta = 1) against fp64 dot products; the plan must be the paired one."""
+    g = torch.Generator(device="cuda").manual_seed(M + N_out + K_in)
+    rng = np.random.default_rng(N_out + K_in)
+    dy = (torch.randn(M, N_out, device="cuda", generator=g) * 0.5).to(torch.bfloat16)
+    x = (torch.randn(M, K_in, device="cuda", generator=g) * 0.5).to(torch.bfloat16)
+    W = (torch.randn(N_out, K_in, device="cuda", generator=g) * 0.5).to(torch.bfloat16)
+    G = torch.full((N_out, K_in), 2.0, device="cuda")
+    dx = torch.empty(M, K_in, device="cuda", dtype=torch.bfloat16)
+    ck(lib.paci_op_gemm_backward_pair(pb.BF16, M, N_out, K_in, dy.data_ptr(), N_out, x.data_ptr(), K_in, W.data_ptr(), K_in,
+                                      G.data_ptr(), K_in, dx.data_ptr(), K_in, S0()))
+    plan = pb.gemm_last_plan()
+    assert plan["range_mode"] == 2 and plan["grid"] == 148, plan               # the shared, water-filled grid
+    torch.cuda.synchronize()
+    rows = torch.from_numpy(np.unique(np.concatenate([rng.integers(0, M, 12), [0, 255, 256, M - 1]]))).cuda()
+    ref = host(dy[rows]) @ host(W)
+    got = host(dx[rows])
+    assert max(rel_l2(got[i], ref[i]) for i in range(len(rows))) < 5e-3
+    grow = torch.from_numpy(np.unique(np.concatenate([rng.integers(0, N_out, 12), [0, 255, 256, N_out - 1]]))).cuda()
+    gref = host(dy[:, grow]).T @ host(x) + 2.0
+    ggot = host(G[grow])
+    assert max(rel_l2(ggot[i], gref[i]) for i in range(len(grow))) < 1e-4

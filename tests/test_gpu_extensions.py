@@ -253,8 +253,8 @@ def test_counters_survive_a_checkpoint_and_resume():
     lc = [step(c, m) for m in range(5, 7)]
     assert np.allclose(lb + lc, la, rtol=1e-5)         # fp32 atomics: equal up to summation order (R21)
     assert c.version == a.version == 3
-    for n in names:
-        assert rel_l2(c.read(n), a.read(n)) < 1e-4, n
+    for n in names:    # (the key bias has a zero gradient: Adam turns its rounding noise into +-lr steps)
+        assert rel_l2(c.read(n), a.read(n)) < (1e-4 if not n.endswith("attn.bqkv") else 5e-2), n
     # ... and a resumed stage that does NOT restore the counters takes a visibly different step (t = 1 bias correction)
     d = pb.Stage(pb.make_config(0, 1, 1, D, H, T, mu, k, V, pb.FP32))
     for w, dd in saved.items():

@@ -291,3 +291,28 @@ def test_out_of_range_token_ids_are_clamped_not_dereferenced():
     got = host(x)[0]
     for t, want in enumerate([0, 49, 49, 0, 7, 49, 3, 4]):
         assert np.array_equal(got[t], wte[want].astype(np.float64))
+
+
+@pytest.mark.parametrize("dtype", BOTH)
+@pytest.mark.parametrize("M,N_out,K_in", [(130, 72, 40), (384, 256, 512), (300, 520, 264), (1024, 1024, 256)])
+def test_gemm_backward_pair(dtype, M, N_out, K_in):
+    """Rows a13 + a14 in ONE launch (bf16): dx = dy W with the current W (Eq. 1) and G_W += dy^T x (Alg. 1 line 13),
+    the wgrad's k-blocks poured over the CTA pairs on top of the dgrad's tiles; G pre-filled and the call repeated
+    (beta = 1), ragged M / N / K tails, row strides wider than the extents."""
+    rng = np.random.default_rng(M + N_out + K_in)
+    dy, x, W = rng.standard_normal((M, N_out)), rng.standard_normal((M, K_in)), rng.standard_normal((N_out, K_in)) * 0.3
+    dyr, xr, Wr = rounded(dy, dtype), rounded(x, dtype), rounded(W, dtype)
+    dx_ref, dW_ref, _ = model.linear_bwd(dyr, xr, Wr)
+    def padded(a):
+        ld = (a.shape[1] + 7) // 8 * 8 + 8
+        buf = np.full((a.shape[0], ld), 9.0)
+        buf[:, :a.shape[1]] = a
+        return dev(buf, dtype), ld
+    dyd, ld_dy = padded(dy); xd, ld_x = padded(x); Wd, ld_w = padded(W)
+    G = torch.full((N_out, K_in), 3.0, device="cuda")
+    dx = torch.empty(M, K_in, device="cuda", dtype=DT[dtype])
+    for _ in range(2):
+        ck(lib.paci_op_gemm_backward_pair(dtype, M, N_out, K_in, dyd.data_ptr(), ld_dy, xd.data_ptr(), ld_x, Wd.data_ptr(),
+                                          ld_w, G.data_ptr(), K_in, dx.data_ptr(), K_in, S0))
+    assert rel_l2(host(dx), dx_ref) < TOL[dtype] / 4
+    assert rel_l2(host(G) - 3.0, 2 * dW_ref) < (1e-5 if dtype == pb.FP32 else 1e-4)
