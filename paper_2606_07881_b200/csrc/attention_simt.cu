@@ -27,6 +27,7 @@ __device__ __forceinline__ float block_reduce(float v, bool is_max, float* red) 
 template <typename T>
 __global__ void __launch_bounds__(128) attn_fwd_simt_kernel(int T_, int H, int dh, const T* __restrict__ qkv,
                                                             T* __restrict__ o, float* __restrict__ lse) {
+  PACI_PDL_SYNC;
   extern __shared__ float sm[];     // q[dh] | s[T]
   __shared__ float red[4];
   float* q = sm;
@@ -69,6 +70,7 @@ __global__ void __launch_bounds__(128) attn_bwd_dq_simt_kernel(int T_, int H, in
                                                                const T* __restrict__ qkv, const T* __restrict__ o,
                                                                const float* __restrict__ lse, T* __restrict__ dqkv,
                                                                float* __restrict__ delta) {
+  PACI_PDL_SYNC;
   extern __shared__ float sm[];     // q[dh] | do[dh] | ds[T]
   __shared__ float red[4];
   float* q = sm;
@@ -114,6 +116,7 @@ __global__ void __launch_bounds__(128) attn_bwd_dkv_simt_kernel(int T_, int H, i
                                                                 const float* __restrict__ lse,
                                                                 const float* __restrict__ delta,
                                                                 T* __restrict__ dqkv) {
+  PACI_PDL_SYNC;
   extern __shared__ float sm[];     // k[dh] | v[dh] | P[T] | ds[T]
   float* k = sm;
   float* v = sm + dh;

@@ -129,6 +129,7 @@ attn_fwd_tc_kernel(const __grid_constant__ CUtensorMap tm, int T, int H, bf16* _
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  PACI_PDL_SYNC;
   const uint32_t tS = tmem_base, tO = tmem_base + 128, tP = tmem_base + 192;   // P: 128 keys as bf16 = 64 columns
 
   if (warp == 0) {
@@ -378,6 +379,7 @@ attn_bwd_tc_kernel(const __grid_constant__ CUtensorMap mX0, const __grid_constan
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  PACI_PDL_SYNC;
   const uint32_t tT0 = tmem_base, tT1 = tmem_base + 64, tA0 = tmem_base + 128, tA1 = tmem_base + 192;
   const uint32_t tE = tmem_base + 128;                   // DQ only (no dV accumulator there): dS as bf16, 32 columns
 
@@ -703,6 +705,7 @@ __global__ void __launch_bounds__(256) attn_delta_tc_kernel(size_t n_vec, int T,
                                                             const bf16* __restrict__ o, const float* __restrict__ lse,
                                                             float* __restrict__ delta, float* __restrict__ lse2,
                                                             int* __restrict__ work_counters) {
+  PACI_PDL_SYNC;
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < 2) work_counters[i] = 0;                        // item counters of the two persistent backward kernels
   float acc = 0.f;

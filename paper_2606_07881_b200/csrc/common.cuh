@@ -27,12 +27,42 @@ int fail(int code, const char* fmt, ...);
                           cudaGetErrorString(e__));                                     \
   } while (0)
 
+// Programmatic dependent launch (PDL).  Every kernel of the library is launched with
+// cudaLaunchAttributeProgrammaticStreamSerialization and starts with PACI_PDL_SYNC (after its own on-chip set-up:
+// barrier init, TMEM allocation, descriptor prefetch): `griddepcontrol.wait` blocks until the previous kernel of the
+// stream has COMPLETED and its memory is visible, so no kernel touches global memory early; `launch_dependents` then
+// lets the NEXT kernel of the stream be scheduled onto SMs as they free up, where it runs its set-up and parks in its
+// own wait.  What is hidden is the launch latency and the prologue, never a data dependency.
+#ifndef PACI_NO_PDL
+#define PACI_PDL_SYNC do { asm volatile("griddepcontrol.wait;" ::: "memory"); \
+                           asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); } while (0)
+#define PACI_PDL_ATTR 1
+#else
+#define PACI_PDL_SYNC do {} while (0)
+#define PACI_PDL_ATTR 0
+#endif
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream,
+                                 Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = PACI_PDL_ATTR;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kernel, static_cast<KArgs>(args)...);
+}
+
 // every kernel launch goes through this so that paci_launch_count() is exact
 #define PACI_LAUNCH(kernel, grid, block, smem, stream, ...)                             \
   do {                                                                                  \
-    kernel<<<(grid), (block), (smem), (stream)>>>(__VA_ARGS__);                         \
+    PACI_CUDA_OK(::paci::launch_kernel(kernel, dim3(grid), dim3(block), (smem), (stream), __VA_ARGS__)); \
     ::paci::g_launches.fetch_add(1, std::memory_order_relaxed);                         \
-    PACI_CUDA_OK(cudaPeekAtLastError());                                                \
   } while (0)
 
 // ---------------------------------------------------------------- dtype traits

@@ -74,6 +74,7 @@ __global__ void __launch_bounds__(256) ln_fwd_kernel(int rows, int D, const T* _
                                                      const float* __restrict__ b, T* __restrict__ xsum,
                                                      T* __restrict__ y, float* __restrict__ mean_out,
                                                      float* __restrict__ rstd_out) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   const int lane = threadIdx.x & 31;
   const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -148,6 +149,7 @@ __global__ void __launch_bounds__((SETS * LNQ_R + 1) * 32, 1) ln_fwd_pipe_kernel
                                                                                 T* __restrict__ xsum, T* __restrict__ y,
                                                                                 float* __restrict__ mean_out,
                                                                                 float* __restrict__ rstd_out) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N, NV = 4, D = NV * 32 * V;
   constexpr uint32_t RB = D * sizeof(T), TB = LNQ_R * RB, STAGE = 2 * TB;
   extern __shared__ __align__(128) uint8_t lnq_smem[];
@@ -307,6 +309,7 @@ __global__ void __launch_bounds__(256, 3) ln_bwd_dx_kernel(int rows, int D, cons
                                                            const float* __restrict__ rstd,
                                                            const float* __restrict__ g, const T* __restrict__ dres,
                                                            T* __restrict__ dx) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   const int lane = threadIdx.x & 31;
   const int row = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -377,6 +380,7 @@ __global__ void __launch_bounds__(LNC_TX * LNC_TY, 1) ln_bwd_cols_kernel(int row
                                                                        const float* __restrict__ rstd,
                                                                        const T* __restrict__ dx, float* __restrict__ Gg,
                                                                        float* __restrict__ Gb, float* __restrict__ Gcol) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   __shared__ __align__(16) float red[3][LNC_TX * V];
   const int tx = threadIdx.x, ty = threadIdx.y;
@@ -456,6 +460,7 @@ __global__ void __launch_bounds__(NW * 32) ln_bwd_fused_kernel(int rows, int D, 
                                                                const float* __restrict__ g, const T* __restrict__ dres,
                                                                T* __restrict__ dx, float* __restrict__ Gg,
                                                                float* __restrict__ Gb, float* __restrict__ Gcol) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   __shared__ float part[2][LNF_R][2][NW];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -564,6 +569,7 @@ __global__ void __launch_bounds__((SETS * NW + 1) * 32, SETS > 1 ? 1 : 2) ln_bwd
                                                                    const float* __restrict__ g, const T* __restrict__ dres,
                                                                    T* __restrict__ dx, float* __restrict__ Gg,
                                                                    float* __restrict__ Gb, float* __restrict__ Gcol) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   constexpr uint32_t RB = NW * 32 * V * sizeof(T);        // bytes of one row
   constexpr uint32_t TB = LNP_R * RB;                     // one tensor's share of a stage
@@ -792,6 +798,7 @@ template <typename T> __device__ __forceinline__ float dgelu_f(float p) {
 
 template <typename T>
 __global__ void __launch_bounds__(256) gelu_fwd_kernel(size_t nvec, const T* __restrict__ p, T* __restrict__ out) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
     float v[V];
@@ -824,6 +831,7 @@ template <typename T, bool GELU>
 __global__ void __launch_bounds__(CS_TX * CS_TY, 2) colslab_kernel(int rows, int cols, const T* __restrict__ a,
                                                                  const T* __restrict__ p, T* __restrict__ out,
                                                                  float* __restrict__ G) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   __shared__ __align__(16) float red[CS_TX * V];
   const int tx = threadIdx.x, ty = threadIdx.y;
@@ -925,6 +933,7 @@ __global__ void __launch_bounds__(256) embed_fwd_kernel(int M, int T_, int D, co
                                                         const float* __restrict__ wte,
                                                         const float* __restrict__ wpe, T* __restrict__ x,
                                                         int vocab, int64_t* __restrict__ err) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   const int nvec = D / V;
   const size_t total = (size_t)M * nvec;
@@ -960,6 +969,7 @@ template <typename T>
 __global__ void __launch_bounds__(256) embed_bwd_wte_kernel(int M, int D, const int32_t* __restrict__ tok,
                                                             const T* __restrict__ dx, float* __restrict__ Gwte,
                                                             int vocab) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   const int nvec = D / V;
   const size_t total = (size_t)M * nvec;
@@ -978,6 +988,7 @@ __global__ void __launch_bounds__(256) embed_bwd_wte_kernel(int M, int D, const 
 template <typename T>
 __global__ void __launch_bounds__(256) embed_bwd_wpe_kernel(int mu, int T_, int D, const T* __restrict__ dx,
                                                             float* __restrict__ Gwpe) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   const int nvec = D / V;
   const size_t total = (size_t)T_ * nvec;
@@ -1030,6 +1041,7 @@ template <typename T>
 __global__ void __launch_bounds__(512) softmax_ce_kernel(int rows, int V_, int ldz, T* __restrict__ z,
                                                          const int32_t* __restrict__ tgt,
                                                          float* __restrict__ loss, int64_t* __restrict__ err) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   __shared__ float red_m[16], red_s[16];
   __shared__ float sh_max, sh_sum;
@@ -1108,6 +1120,7 @@ __global__ void __launch_bounds__(256) adamw_kernel(size_t n4, size_t n4_decay, 
                                                     float inv_k, float lr, float beta1, float beta2, float eps,
                                                     float decay_mul, float inv_bc1, float inv_bc2,
                                                     int64_t* version_word) {
+  PACI_PDL_SYNC;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += (size_t)gridDim.x * blockDim.x) {
     float4 W = w[i], Mv = m[i], Vv = v[i], Gv = G[i];
     const float dm = i < n4_decay ? decay_mul : 1.f;
@@ -1151,6 +1164,7 @@ int adamw(size_t n, size_t n_decay, float* w, float* m, float* v, float* G, void
 }
 
 __global__ void cast_shadow_kernel(size_t n, const float* __restrict__ w, bf16* __restrict__ sh) {
+  PACI_PDL_SYNC;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
     sh[i] = __float2bfloat16_rn(w[i]);
 }
@@ -1183,6 +1197,7 @@ template <typename T>
 __global__ void __launch_bounds__(256) dropout_kernel(size_t nvec, const T* __restrict__ x, T* __restrict__ out,
                                                       uint32_t thresh, float scale, uint32_t k0, uint32_t k1,
                                                       uint32_t mb, uint32_t site) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
     float v[V];
@@ -1221,6 +1236,7 @@ int dropout(int dtype, size_t n, const void* x, void* out, float p, uint64_t see
 template <typename T>
 __global__ void __launch_bounds__(256) add_vec_kernel(size_t nvec, const T* __restrict__ a, const T* __restrict__ b,
                                                       T* __restrict__ out) {
+  PACI_PDL_SYNC;
   constexpr int V = Vec<T>::N;
   for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
     float x[V];
@@ -1248,7 +1264,8 @@ int add_vec(int dtype, size_t n, const void* a, const void* b, void* out, cudaSt
   return PACI_OK;
 }
 
-__global__ void stamp_kernel(const int64_t* version_word, int64_t* dst) { *dst = *version_word; }
+__global__ void stamp_kernel(const int64_t* version_word, int64_t* dst) {
+  PACI_PDL_SYNC; *dst = *version_word; }
 int stamp_version(const int64_t* version_word, int64_t* dst, cudaStream_t s) {
   PACI_LAUNCH(stamp_kernel, 1, 1, 0, s, version_word, dst);
   return PACI_OK;
@@ -1256,6 +1273,7 @@ int stamp_version(const int64_t* version_word, int64_t* dst, cudaStream_t s) {
 
 __global__ void split_tokens_kernel(int mu, int T_, const int32_t* __restrict__ src, int32_t* __restrict__ inp,
                                     int32_t* __restrict__ tgt) {
+  PACI_PDL_SYNC;
   const int n = mu * T_;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
     const int b = i / T_, t = i % T_;

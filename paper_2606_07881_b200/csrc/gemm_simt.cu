@@ -14,6 +14,7 @@ __global__ void __launch_bounds__(256) gemm_simt_kernel(int M, int N, int K, con
                                                         long a_sk, const T* __restrict__ B, long b_sn, long b_sk,
                                                         const float* __restrict__ bias, void* __restrict__ Cv,
                                                         int ldc, int accum) {
+  PACI_PDL_SYNC;
   constexpr int BM = 64, BN = 64, BK = 16;
   __shared__ float As[BK][BM + 4];
   __shared__ float Bs[BK][BN + 4];

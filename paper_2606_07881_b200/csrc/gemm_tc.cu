@@ -167,6 +167,7 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
   if (warp == 1) asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  PACI_PDL_SYNC;                                       // set-up above overlaps the previous kernel's tail
 
   const int worker = (int)(blockIdx.x >> 1);
   const int n_workers = (int)(gridDim.x >> 1);
@@ -474,13 +475,15 @@ int launch(const Maps& maps, const Params& p, int grid, cudaStream_t s) {
   cfg.blockDim = dim3(NUM_THREADS);
   cfg.dynamicSmemBytes = SMEM;
   cfg.stream = s;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = 2;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
+  attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[1].val.programmaticStreamSerializationAllowed = PACI_PDL_ATTR;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = 2;
   PACI_CUDA_OK(cudaLaunchKernelEx(&cfg, kern, maps, p));
   g_launches.fetch_add(1, std::memory_order_relaxed);
   return PACI_OK;

@@ -158,7 +158,7 @@ def test_embedding_fwd_bwd_zipf(dtype):
 
 
 @pytest.mark.parametrize("dtype", BOTH)
-@pytest.mark.parametrize("rows,V", [(19, 256), (33, 50257)])
+@pytest.mark.parametrize("rows,V", [(19, 256), (33, 50257), (700, 5000)])   # 700 rows: every persistent block wraps its two row buffers
 def test_softmax_cross_entropy(dtype, rows, V):
     rng = np.random.default_rng(V)
     ldz = (V + 63) // 64 * 64
