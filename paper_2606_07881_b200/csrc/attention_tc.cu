@@ -742,27 +742,17 @@ int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, co
   if ((rc = make_tensor_map(&q64, qkv, 3 * (uint64_t)D, rows, 3 * (uint64_t)D, 64, 64, 2))) return rc;
   if ((rc = make_tensor_map(&d128, dout, (uint64_t)D, rows, (uint64_t)D, 64, 128, 2))) return rc;
   if ((rc = make_tensor_map(&d64, dout, (uint64_t)D, rows, (uint64_t)D, 64, 64, 2))) return rc;
-  static bool attr_set = false;
-  if (!attr_set) {
-    PACI_CUDA_OK(cudaFuncSetAttribute(attn_bwd_tc_kernel<true, BWD_EW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bwd_smem(true)));
-    PACI_CUDA_OK(cudaFuncSetAttribute(attn_bwd_tc_kernel<false, BWD_EW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bwd_smem(false)));
-    attr_set = true;
-  }
+  { int rc_ = set_max_dynamic_smem((const void*)attn_bwd_tc_kernel<true, BWD_EW>, (int)bwd_smem(true)); if (rc_) return rc_; }
+  { int rc_ = set_max_dynamic_smem((const void*)attn_bwd_tc_kernel<false, BWD_EW>, (int)bwd_smem(false)); if (rc_) return rc_; }
   float* delta = scratch;
   float* lse2 = scratch + (size_t)mu * H * T;
   int* counters = reinterpret_cast<int*>(scratch + 2 * (size_t)mu * H * T);
   const size_t n_vec = (size_t)mu * T * D / 8;
   PACI_LAUNCH(attn_delta_tc_kernel, ceil_div((long long)n_vec, 256), 256, 0, s, n_vec, T, H, (const bf16*)dout,
               (const bf16*)o, lse, delta, lse2, counters);
-  static int n_sm = 0;
-  if (n_sm == 0) {
-    int dev = 0;
-    PACI_CUDA_OK(cudaGetDevice(&dev));
-    PACI_CUDA_OK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-  }
+  const int n_sm = num_sms();
   const int items = (T / 128) * H * mu;
-  static const int per_sm = getenv("PACI_ATTN_CTAS") ? atoi(getenv("PACI_ATTN_CTAS")) : 2;
-  const int grid = (per_sm <= 0 || items < per_sm * n_sm) ? items : per_sm * n_sm;   // persistent: two CTAs per SM
+  const int grid = items < 2 * n_sm ? items : 2 * n_sm;   // persistent: two CTAs per SM
   // dK, dV: stationary K_j, V_j (qkv, 128-row boxes); streamed Q_i (qkv), dO_i (dout), 64-row boxes
   PACI_LAUNCH((attn_bwd_tc_kernel<true, BWD_EW>), grid, BWD_THREADS, bwd_smem(true), s, q128, q128, q64, d64, T, H, mu, lse2, delta,
               (bf16*)dqkv, Gbias, counters);
@@ -777,11 +767,7 @@ int attention_fwd_tc(int mu, int T, int H, const void* qkv, void* o, float* lse,
   CUtensorMap tm;
   int rc = make_tensor_map(&tm, qkv, 3 * (uint64_t)D, (uint64_t)mu * T, 3 * (uint64_t)D, 64, 128, 2);
   if (rc) return rc;
-  static bool attr_set = false;
-  if (!attr_set) {
-    PACI_CUDA_OK(cudaFuncSetAttribute(attn_fwd_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FWD_SMEM));
-    attr_set = true;
-  }
+  { int rc_ = set_max_dynamic_smem((const void*)attn_fwd_tc_kernel, (int)FWD_SMEM); if (rc_) return rc_; }
   const int grid = (T / 128) * H * mu;
   PACI_LAUNCH(attn_fwd_tc_kernel, grid, FWD_THREADS, FWD_SMEM, s, tm, T, H, (bf16*)o, lse);
   return PACI_OK;
