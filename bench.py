@@ -229,16 +229,99 @@ def run_reference(args, c, name):
 
 
 # ------------------------------------------------------------------------------------ CUDA leg
-def build_pipeline(pb, c, device):
+def build_pipeline(pb, c, device, layers=None, checkpoint=0):
+    """layers: blocks per stage (default: the equal split of BASELINE.json, c['L'] each)."""
     import synth
     dt = pb.BF16 if c["dtype"] == "bf16" else pb.FP32
-    stages = []
+    layers = list(layers) if layers is not None else [c["L"]] * c["S"]
+    stages, first = [], 0
     for s in range(c["S"]):
-        st = pb.Stage(pb.make_config(s, c["S"], c["L"], c["D"], c["H"], c["T"], c["mu"], c["k"], c["V"], dt),
-                      device=device)
-        st.load_params(synth.stage_params(SEED, s, c["S"], c["L"], c["D"], c["V"], c["T"]))
+        st = pb.Stage(pb.make_config(s, c["S"], layers[s], c["D"], c["H"], c["T"], c["mu"], c["k"], c["V"], dt,
+                                     checkpoint=checkpoint), device=device)
+        st.load_params(synth.stage_params(SEED, s, c["S"], layers[s], c["D"], c["V"], c["T"], first_block=first))
+        first += layers[s]
         stages.append(st)
     return stages, pb.Pipeline(stages)
+
+
+def free_pipeline(torch, stages, pipe):
+    pipe.close()
+    for st in stages:
+        st.close()
+    stages.clear()
+    torch.cuda.empty_cache()
+
+
+def timed_steps(pipe, tok_dev, lr, first, steps, S, tokens_per_step):
+    """Device time of `steps` pipeline steps on resident tokens -> (tokens/s per stage step, ms per step)."""
+    ms = 0.0
+    for i in range(steps):
+        ms += pipe.run(tok_dev[first + i], lr, want_delta=False)["elapsed_ms"]
+    return S * tokens_per_step * steps / (ms * 1e-3), ms / steps
+
+
+def partition_profile(pb, c, per_stage):
+    """Per-layer profile for App. D.5 from THIS build's own measurements: the layers are the L*S
+    transformer blocks (the embedding grouped with the first) plus the final layer that computes the
+    loss.  t_l = forward time (the paper's proxy), s_l = bytes of parameters + gradient accumulator + optimizer state
+    (+ bf16 shadow), a_l = bytes stashed for backward per micro-batch (from paci_stage_workspace_bytes)."""
+    import ctypes as C
+    S, L, D, H, T, mu, V, k = c["S"], c["L"], c["D"], c["H"], c["T"], c["mu"], c["V"], c["k"]
+    dt = pb.BF16 if c["dtype"] == "bf16" else pb.FP32
+
+    def ws(s_idx, n_layers, emb, head):
+        cfg = pb.make_config(s_idx, 2, n_layers, D, H, T, mu, k, V, dt, has_embedding=emb, has_head=head)
+        return pb.lib.paci_stage_workspace_bytes(C.byref(cfg))
+
+    def nparams(n_layers, emb, head):
+        cfg = pb.make_config(0, 2, n_layers, D, H, T, mu, k, V, dt, has_embedding=emb, has_head=head)
+        return pb.lib.paci_stage_param_count(C.byref(cfg))
+    a_block = (ws(0, 2, False, False) - ws(1, 2, False, False)) - (ws(0, 1, False, False) - ws(1, 1, False, False))
+    a_head = ws(0, 0, False, True) - ws(1, 0, False, True)
+    bpp = 18.0 if dt == pb.BF16 else 16.0
+    s_block = bpp * (nparams(2, False, False) - nparams(1, False, False))
+    s_head = bpp * nparams(0, False, True)
+    s_emb = bpp * (nparams(1, True, False) - nparams(1, False, False))
+    t_block = per_stage[1 if S >= 3 else 0]["t_fwd_ms"] / L
+    t_emb = max(per_stage[0]["t_fwd_ms"] - L * t_block, 0.0) if S > 1 else 0.0
+    t_head = max(per_stage[S - 1]["t_fwd_ms"] - L * t_block, 0.0)
+    n_blocks = L * S
+    t = [t_block] * n_blocks + [t_head]
+    s_ = [s_block] * n_blocks + [s_head]
+    a = [float(a_block)] * n_blocks + [float(a_head)]
+    t[0] += t_emb
+    s_[0] += s_emb
+    return t, s_, a
+
+
+def run_partition(pb, torch, c, stages, pipe, per_stage, tok_dev, lr, device, steps=2):
+    """--partition auto: App. D.5 (Eq. 12-15) fed by this build's own per-layer profile; the S stages
+    then hold unequal numbers of blocks.  One GPU serialises the emulated stages, so the gain shows where the paper
+    puts it: the slowest stage bounds a pipeline's steady-state throughput (PAPER.md:460 'bottle-necked by the slowest
+    stage')."""
+    S, L, mu, T, k = c["S"], c["L"], c["mu"], c["T"], c["k"]
+    t, s_, a = partition_profile(pb, c, per_stage)
+    budget = 180e9 / S                     # the S emulated stages share one 180 GB B200
+    part = pb.partition(t, s_, a, S, budget)
+    cuts = part["cuts"]
+    layers = [cuts[j + 1] - cuts[j] for j in range(S)]
+    layers[-1] -= 1                        # the last group's final layer is the head, not a block
+    free_pipeline(torch, stages, pipe)
+    stages2, pipe2 = build_pipeline(pb, c, device, layers=layers)
+    pipe2.run(tok_dev[0], lr, want_delta=False)
+    value, ms = timed_steps(pipe2, tok_dev, lr, 1, steps, S, c["n_micro"] * mu * T)
+    st2 = per_stage_times(pb, torch, dict(c), stages2, reps=2)
+    free_pipeline(torch, stages2, pipe2)
+    slow = lambda ps: max(p["t_fwd_ms"] + p["t_bwd_ms"] + p["t_step_ms"] / k for p in ps)
+    return {"profile": {"t_block_ms": t[1], "t_first_ms": t[0], "t_head_ms": t[-1], "s_block_bytes": s_[1],
+                        "a_block_bytes": a[1], "a_head_bytes": a[-1], "budget_bytes": budget},
+            "cuts": cuts, "blocks_per_stage": layers, "fallback": part["fallback"],
+            "predicted_max_stage_fwd_ms": part["max_time"],
+            "equal_split": {"blocks_per_stage": [L] * S, "slowest_stage_ms": slow(per_stage),
+                            "pipeline_tokens_per_s_bound": mu * T / (slow(per_stage) * 1e-3)},
+            "partitioned": {"slowest_stage_ms": slow(st2), "pipeline_tokens_per_s_bound": mu * T / (slow(st2) * 1e-3),
+                            "tokens_per_s_per_stage_step_one_gpu": value, "ms_per_step_one_gpu": ms,
+                            "per_stage": st2}}
 
 
 def per_stage_times(pb, torch, c, stages, reps=3):
@@ -290,6 +373,7 @@ def run_ours(args, c, name):
     S, mu, T, n_micro, k = c["S"], c["mu"], c["T"], c["n_micro"], c["k"]
     tokens_per_step = n_micro * mu * T
     stages, pipe = build_pipeline(pb, c, device)
+    ws_total = sum(st.workspace_bytes for st in stages)
     n_batches = args.warmup + 2 * args.steps
     tok_host = synth.tokens(SEED + rank, n_batches * n_micro, mu, T, c["V"], c["dist"])
     tok_host = tok_host.reshape(n_batches, n_micro, mu, T + 1)
@@ -373,12 +457,27 @@ def run_ours(args, c, name):
                 "sampled_launches": g_n, "sample_stride": args.sample_stride}
 
     stage_times = per_stage_times(pb, torch, c, stages) if not args.no_stage_times else None
+    extras = {}
+    if args.partition == "auto" and stage_times is not None and S > 1:
+        extras["partition"] = run_partition(pb, torch, c, stages, pipe, stage_times, tok_dev, lr, device)
+    else:
+        free_pipeline(torch, stages, pipe)
+    if not args.no_extras:
+        # activation-checkpointed PACI on the same workload: the stash shrinks to the stage input and
+        # every backward first recomputes its stage's forward under the current weights
+        st_ck, pipe_ck = build_pipeline(pb, c, device, checkpoint=1)
+        pipe_ck.run(tok_dev[0], lr, want_delta=False)
+        v_ck, ms_ck = timed_steps(pipe_ck, tok_dev, lr, 1, min(2, args.steps), S, tokens_per_step)
+        ws_ck = sum(st.workspace_bytes for st in st_ck)
+        free_pipeline(torch, st_ck, pipe_ck)
+        extras["checkpointed_paci"] = {"value": v_ck, "unit": UNIT, "ms_per_step": ms_ck, "stage_workspace_bytes": ws_ck,
+                                       "note": "checkpoint=1: backward = recompute under current weights + differentiate"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": c["dtype"], "data": "synthetic",
             "config": {"workload": workload_name(name, c), "n_stages": S, "tokens_per_step": tokens_per_step,
-                       "stage_steps_per_step": S * n_micro,
+                       "stage_steps_per_step": S * n_micro, "stage_workspace_bytes": ws_total,
                        "l2": "inputs larger than L2 (each step streams > 20 GB of weights and stashed activations)",
                        "parallelism": "replicas only" if world > 1 else "1 GPU, S emulated stages on per-stage streams",
                        "gemm_backend": "tcgen05"},
@@ -392,8 +491,10 @@ def run_ours(args, c, name):
             "max_crossed_updates": delta_max, "mean_loss_per_step": losses}
     if stage_times is not None:
         line["per_stage"] = stage_times
+    if extras:
+        line["extras"] = extras
     if world == 1 and not args.no_cpu_baseline:
-        val, info = oracle_sample(c, 1, 0)
+        val, info = oracle_sample(c, 3, 1)                # 3 timed oracle steps after 1 warm-up step (~25 s of host time)
         line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": info["cores"], "kind": "oracle",
                                 "sample": info["sample"]}
         try:
@@ -472,6 +573,10 @@ def main():
                     help="time every n-th library op with CUDA events; a sampled op runs alone on the GPU")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-stage-times", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the checkpointed-PACI extra measurement")
+    ap.add_argument("--partition", default="equal", choices=["equal", "auto"],
+                    help="auto: also run App. D.5's partitioner on this build's own per-layer profile and report "
+                         "the partitioned pipeline as an EXTRA (the headline stays on BASELINE.json's equal split)")
     ap.add_argument("--k-sweep", action="store_true", help="BASELINE.json configs[3]: k in {1,2,4,8}, PACI vs flush")
     args = ap.parse_args()
     c = CONFIGS[args.config]

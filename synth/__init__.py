@@ -76,7 +76,7 @@ def param_shape(name: str, d_model: int, vocab: int, seq_len: int):
 
 
 def stage_params(seed: int, stage_index: int, n_stages: int, n_layers: int, d_model: int, vocab: int,
-                 seq_len: int, perturbed: bool = False) -> dict:
+                 seq_len: int, perturbed: bool = False, first_block: int | None = None) -> dict:
     """fp32 initial parameters of one stage (dict name -> float32 array).
 
     Matrices, wte, wpe ~ N(0, 0.02); biases 0; LN gain 1, LN bias 0.
@@ -96,7 +96,8 @@ def stage_params(seed: int, stage_index: int, n_stages: int, n_layers: int, d_mo
             stream = f"param/{name}"
         else:  # transformer block l of this stage = global block stage_index*n_layers + l
             l = int(name.split(".")[1])
-            stream = f"param/h.{stage_index * n_layers + l}." + name.split(".", 2)[2]
+            base = stage_index * n_layers if first_block is None else first_block   # unequal splits name their first block
+            stream = f"param/h.{base + l}." + name.split(".", 2)[2]
         rng = _rng(seed, stream)
         leaf = name.rsplit(".", 1)[-1]
         if len(shape) == 2:

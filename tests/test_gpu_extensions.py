@@ -284,3 +284,27 @@ def test_delta_log_survives_ring_recycling_with_reused_ids():
     torch.cuda.synchronize()
     assert st.device_stamps(n - 1) == (0, 0)
     st.close()
+
+
+def test_stage_worker_drives_a_real_stage_single_rank():
+    """The stage-per-GPU event loop (8(f) f-1) with binding.Stage as its stage object, world size 1 (one stage holding
+    both ends, no neighbour): the loop's forward / backward / update order must reproduce the oracle's S = 1 run.  The
+    multi-rank transport is covered on CPU over gloo (tests/test_stage_per_gpu.py)."""
+    from paper_2606_07881_b200.stage_per_gpu import StageWorker
+    V, D, H, T, mu, L, k, n, lr = 256, 64, 4, 32, 2, 1, 2, 6, 2e-3
+    specs, params, stages = _build(pb.FP32, 1, L, D, H, T, mu, V, k, seed=51)
+    tok = synth.tokens(51, n, mu, T, V, "uniform")
+    ref = opipe.run_pipeline(specs, params, tok, k, lr)
+    inp = [torch.from_numpy(tok[m, :, :-1].copy()).cuda() for m in range(n)]
+    tgt = [torch.from_numpy(tok[m, :, 1:].copy()).cuda() for m in range(n)]
+    losses = [torch.zeros(1, device="cuda") for _ in range(n)]
+    w = StageWorker(stages[0], 0, 1, lambda: torch.empty(mu, T, D, device="cuda"), None)
+    rep = w.run(n, lr, inputs=lambda m: inp[m], targets=lambda m: tgt[m], losses=losses)
+    torch.cuda.synchronize()
+    assert rep["delta"] == ref["delta"][0] == [0] * n and rep["version"] == ref["version"][0] == n // k
+    assert [e for e in rep["events"] if e[0] == "U"] == [("U", 1), ("U", 2), ("U", 3)]
+    got = np.array([x.item() for x in losses])
+    assert np.max(np.abs(got - np.array(ref["losses"])) / np.array(ref["losses"])) < 2e-5
+    for name, th in ref["opt"][0].theta.items():
+        if not name.endswith("attn.bqkv"):
+            assert rel_l2(stages[0].read(name), th) < WTOL[pb.FP32], name
