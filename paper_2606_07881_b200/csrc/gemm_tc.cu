@@ -563,10 +563,7 @@ int gemm_tc_multi(const GemmDesc* d, int n, cudaStream_t s) {
     if (rc) return rc;
   }
   if (n == 1) { maps.a[1] = maps.a[0]; maps.b[1] = maps.b[0]; maps.c[1] = maps.c[0]; if (!d[0].gelu_out) maps.c2 = maps.c[0]; }
-#ifndef PACI_GEMM_WORKERS_DIV
-#define PACI_GEMM_WORKERS_DIV 1
-#endif
-  const int workers = std::min(std::max(1, num_sms() / 2 / PACI_GEMM_WORKERS_DIV), MAX_WORKERS);
+  const int workers = std::min(std::max(1, num_sms() / 2), MAX_WORKERS);
   int grid;
   if (n == 1) {
     Prob& pr = p.pr[0];
