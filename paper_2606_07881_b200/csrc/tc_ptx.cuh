@@ -101,8 +101,12 @@ __device__ __forceinline__ uint32_t mapa_rank(uint32_t saddr, uint32_t rank) {  
 __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+// Arrive on a barrier of (possibly) the other CTA of the pair.  Default semantics (.release.cta), NOT .release.cluster:
+// what the arrival publishes is "this warp's tcgen05.ld of the accumulator have completed" (tcgen05.wait::ld +
+// tcgen05.fence::before_thread_sync), no generic-proxy memory; the cluster-scope release compiled to a fence that
+// cost the epilogue warps ~2500 cycles per tile (a third of their time per tile, measured with clock64).
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_addr) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
 // TMA load issued by either CTA of the pair; the bytes are counted on the LEADER's mbarrier (cluster address)
 __device__ __forceinline__ void tma_load_2d_pair(void* dst, const CUtensorMap* map, uint32_t leader_bar, int c0,
