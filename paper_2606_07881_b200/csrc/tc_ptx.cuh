@@ -98,8 +98,11 @@ __device__ __forceinline__ uint32_t mapa_rank(uint32_t saddr, uint32_t rank) {  
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
   return r;
 }
+// Execution barrier of the cluster.  The arrive is RELAXED: none of the four uses in the GEMM publishes generic-proxy
+// memory through it (mbarrier initialisation has its own fence.mbarrier_init.release.cluster, TMEM allocation and
+// tcgen05 traffic are ordered by the tcgen05 fences), and the .release form compiles to MEMBAR.ALL.GPU in every thread.
 __device__ __forceinline__ void cluster_sync_all() {
-  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 // Arrive on a barrier of (possibly) the other CTA of the pair.  Default semantics (.release.cta), NOT .release.cluster:
 // what the arrival publishes is "this warp's tcgen05.ld of the accumulator have completed" (tcgen05.wait::ld +
