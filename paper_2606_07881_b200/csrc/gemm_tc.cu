@@ -167,6 +167,13 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
   if (warp == 5) asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  if (threadIdx.x == 4 * 32) {                         // the descriptors are kernel parameters: fetch them before the wait
+    for (int q = 0; q < p.n_prob; ++q) {
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a[q]) : "memory");
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b[q]) : "memory");
+      asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.c[q]) : "memory");
+    }
+  }
   PACI_PDL_SYNC;                                       // set-up above overlaps the previous kernel's tail
 
   const int worker = (int)(blockIdx.x >> 1);
@@ -177,10 +184,6 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
   // that pace the main loop are never queued behind an epilogue warp of the same sub-partition.
   if (warp == 4) {
     if (lane == 0) {
-      for (int q = 0; q < p.n_prob; ++q) {
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.a[q]) : "memory");
-        asm volatile("prefetch.tensormap [%0];" ::"l"(&maps.b[q]) : "memory");
-      }
       uint32_t stage = 0, phase = 0;
       const uint32_t full0 = mapa_rank(smem_u32(&full[0]), 0);     // the LEADER's full[0]; full[i] is 8 i bytes further
       const uint32_t smem0 = smem_u32(smem);
@@ -322,7 +325,10 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
           }
         }
       } else {
-        const bool gelu = pr.gelu != 0;                // launch-uniform
+        // specialised at compile time on the GELU output: as a runtime flag it put eight branch regions into every
+        // chunk (one per 16-byte store), which kept the plain epilogue's 64 adds and 32 packs from overlapping
+        auto chunks = [&](auto gelu_t) {
+        constexpr bool gelu = decltype(gelu_t)::value;
         int half = 0;
 #pragma unroll 1
         for (int c = 0; c < BLOCK_N; c += 64, half ^= 1) {
@@ -384,6 +390,8 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
             bulk_commit();
           }
         }
+        };
+        if (pr.gelu) chunks(std::true_type{}); else chunks(std::false_type{});
       }
       tc_fence_before();
       __syncwarp();
