@@ -287,6 +287,22 @@ int paci_op_attention_fwd(int dtype, int mu, int T, int H, int dh, const void* q
 int paci_op_attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
                           const void* o, const float* lse, void* dqkv, float* scratch, void* stream);
 size_t paci_op_attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh);
+/* Backward of the attention output projection y = o Wo^T (rows a13 + a14 of that layer, and the prologue of a17):
+ * G_Wo[D, D] += dy^T o (fp32) and d_o[mu T, D] = dy Wo, D = H dh, everything dense row-major (device pointers).
+ * PACI_BF16 with dh = 64, T % 128 = 0 and lse, attn_scratch non-NULL: ONE tcgen05 launch whose dgrad epilogue also
+ * writes, for every (b, h, t), delta = sum_d d_o[b,t,h,d] o[b,t,h,d] (the row term of softmax's backward, from the
+ * ROUNDED d_o it stores) and lse log2(e) into attn_scratch (>= paci_op_attention_bwd_scratch_bytes, the layout
+ * paci_op_attention_bwd uses); *prepared (host int) = 1, and paci_op_attention_bwd_prepared then runs without the
+ * separate delta pass.  Any other case: the plain backward pair, *prepared = 0.  Errors: PACI_EINVAL (NULL prepared,
+ * misaligned pointers), CUDA errors as everywhere. */
+int paci_op_out_proj_backward(int dtype, int mu, int T, int H, int dh, const void* dy, const void* o, const void* Wo,
+                              float* G_Wo, void* d_o, const float* lse, float* attn_scratch, int* prepared,
+                              void* stream);
+/* paci_op_attention_bwd for a scratch that paci_op_out_proj_backward prepared (*prepared = 1) on the same stream with
+ * the same mu, T, H and the d_o passed here as dout.  PACI_BF16 only has such a path; other dtypes ignore the promise
+ * and recompute. */
+int paci_op_attention_bwd_prepared(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
+                                   const void* o, const float* lse, void* dqkv, float* scratch, void* stream);
 /* x = wte[tok] + wpe[pos] (a1);  tok int32 [mu,T]; wte [vocab, D], wpe fp32.  Ids outside [0, vocab) are clamped. */
 int paci_op_embed_fwd(int dtype, int mu, int T, int D, int vocab, const int32_t* tok, const float* wte,
                       const float* wpe, void* x, void* stream);

@@ -84,6 +84,8 @@ SIGNATURES = {
     "paci_op_attention_fwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp]),
     "paci_op_attention_bwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_attention_bwd_scratch_bytes": (_sz, [_i, _i, _i, _i, _i]),
+    "paci_op_out_proj_backward": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "paci_op_attention_bwd_prepared": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_embed_fwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_embed_bwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_dropout": (_i, [_i, _sz, _vp, _vp, _f, C.c_uint64, _i64, C.c_int32, _vp]),

@@ -732,8 +732,10 @@ __global__ void __launch_bounds__(256) attn_delta_tc_kernel(size_t n_vec, int T,
 // delta, lse2 (fp32 [mu, H, T] each) and the two work counters of the persistent kernels
 size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H) { return 2 * (size_t)mu * H * T * sizeof(float) + 64; }
 
+// scratch_prepared: delta and lse2 are already in `scratch` (written by the out-projection dgrad's epilogue,
+// AttnDeltaOut); only the two work counters are reset here.
 int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
-                     void* dqkv, float* scratch, float* Gbias, cudaStream_t s) {
+                     void* dqkv, float* scratch, float* Gbias, int scratch_prepared, cudaStream_t s) {
   const int D = H * DH;
   const uint64_t rows = (uint64_t)mu * T;
   CUtensorMap q128, q64, d128, d64;
@@ -748,8 +750,12 @@ int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, co
   float* lse2 = scratch + (size_t)mu * H * T;
   int* counters = reinterpret_cast<int*>(scratch + 2 * (size_t)mu * H * T);
   const size_t n_vec = (size_t)mu * T * D / 8;
-  PACI_LAUNCH(attn_delta_tc_kernel, ceil_div((long long)n_vec, 256), 256, 0, s, n_vec, T, H, (const bf16*)dout,
-              (const bf16*)o, lse, delta, lse2, counters);
+  if (scratch_prepared) {
+    PACI_CUDA_OK(cudaMemsetAsync(counters, 0, 2 * sizeof(int), s));
+  } else {
+    PACI_LAUNCH(attn_delta_tc_kernel, ceil_div((long long)n_vec, 256), 256, 0, s, n_vec, T, H, (const bf16*)dout,
+                (const bf16*)o, lse, delta, lse2, counters);
+  }
   const int n_sm = num_sms();
   const int items = (T / 128) * H * mu;
   const int grid = items < 2 * n_sm ? items : 2 * n_sm;   // persistent: two CTAs per SM

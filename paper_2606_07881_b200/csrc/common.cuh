@@ -206,6 +206,15 @@ int gemm_simt(int dtype, int layout, int M, int N, int K, const void* A, int lda
 int gemm_tc(int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
             void* C, int ldc, int out_f32_accum, cudaStream_t s, void* gelu_out = nullptr);
 // One GEMM as a value (same fields as gemm()'s arguments).
+// Extra outputs of the out-projection dgrad's epilogue (the prologue of row a17): with C = dO [mu T, H 64] it also
+// writes delta[b,h,t] = sum_d dO[b,t,h,d] O[b,t,h,d] and lse2 = lse log2(e), both fp32 [mu, H, T] -- what the separate
+// attn_delta kernel computes, without re-reading dO.
+struct AttnDeltaOut {
+  const void* o; int ldo;            // attention output O, bf16 [mu T, H 64]
+  const float* lse;                  // [mu, H, T] from the forward
+  float* delta; float* lse2;         // [mu, H, T] each
+  int T, H;
+};
 struct GemmDesc {
   int layout, M, N, K;
   const void* A; int lda;
@@ -214,6 +223,7 @@ struct GemmDesc {
   void* C; int ldc;
   int out_f32_accum;
   void* gelu_out;
+  const AttnDeltaOut* delta;         // NULL unless this is the out-projection dgrad (bf16 only)
 };
 int gemm_tc_multi(const GemmDesc* d, int n, cudaStream_t s);       // n <= 2 problems in ONE persistent launch
 // The backward pair of one linear layer y = x W^T: G_W += dy^T x (wgrad, beta = 1, Alg. 1 line 13) and dx = dy W
@@ -231,7 +241,9 @@ int add_vec(int dtype, size_t n, const void* a, const void* b, void* out, cudaSt
 int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,
                   cudaStream_t s);
 int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv, const void* o,
-                  const float* lse, void* dqkv, float* scratch, float* Gbias, cudaStream_t s);
+                  const float* lse, void* dqkv, float* scratch, float* Gbias, cudaStream_t s, int scratch_prepared = 0);
+int out_proj_backward(int dtype, int mu, int T, int H, int dh, const void* dy, const void* o, const void* Wo,
+                      float* G_Wo, void* d_o, const float* lse, float* attn_scratch, int* prepared, cudaStream_t s);
 size_t attention_bwd_scratch_bytes(int dtype, int mu, int T, int H, int dh);
 int attention_fwd_simt(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,
                        cudaStream_t s);

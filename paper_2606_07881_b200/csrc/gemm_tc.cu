@@ -47,6 +47,7 @@ constexpr int BLOCK_M = 128;
 constexpr int BLOCK_K = 64;
 constexpr int UMMA_K = 16;
 constexpr int NUM_THREADS = 192;
+constexpr float LOG2E_F = 1.4426950408889634f;
 constexpr int EPI_BUFS = 4;                 // staging boxes per epilogue warp: a box is reused only after the TMA store
                                             // issued EPI_BUFS chunks ago has read it (2 buffers left ~0.7 us of store
                                             // latency exposed per chunk); the GELU epilogue uses them as two PAIRS
@@ -66,6 +67,13 @@ struct Prob {
   int a_mn, b_mn;    // operand majors: 0 = K-major, 1 = MN-major
   int accum;         // 0: C is bf16, overwritten, + bias;  1: C is fp32 and the product is ADDED (TMA reduce-add)
   int gelu;          // !accum only: also store gelu(C) through the second map (MLP-up: rows a7 + a8)
+  // !accum, !gelu, out-proj dgrad only (row a17's prologue): C is dO [mu T, H 64]; also emit delta[b,h,t] =
+  // sum_d dO O over the 64 columns of head h (one epilogue chunk) and lse2 = lse log2(e)
+  const void* dl_o;  // attention output O, bf16 [M, N] with row stride dl_ldo; NULL: no delta epilogue
+  const float* dl_lse;
+  float* dl_delta;
+  float* dl_lse2;
+  int dl_ldo, dl_T, dl_H;
   const float* bias;
 };
 struct Params {
@@ -327,8 +335,14 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
       } else {
         // specialised at compile time on the GELU output: as a runtime flag it put eight branch regions into every
         // chunk (one per 16-byte store), which kept the plain epilogue's 64 adds and 32 packs from overlapping
-        auto chunks = [&](auto gelu_t) {
-        constexpr bool gelu = decltype(gelu_t)::value;
+        auto chunks = [&](auto mode_t) {
+        constexpr int mode = decltype(mode_t)::value;
+        constexpr bool gelu = mode == 1, with_delta = mode == 2;
+        // delta epilogue: thread = one row (b, t) of dO; a 64-column chunk is exactly one head
+        const int drow = m0 + q * 32 + lane;
+        const bool drow_ok = with_delta && drow < pr.M;
+        const bf16* dl_orow = reinterpret_cast<const bf16*>(pr.dl_o) + (size_t)(drow_ok ? drow : 0) * pr.dl_ldo + n0;
+        const int dl_b = with_delta ? drow / pr.dl_T : 0, dl_t = with_delta ? drow % pr.dl_T : 0;
         int half = 0;
 #pragma unroll 1
         for (int c = 0; c < BLOCK_N; c += 64, half ^= 1) {
@@ -343,6 +357,13 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
           uint32_t r64[64];                            // both halves of the chunk in flight before one wait
           tmem_ld32_nowait(taddr + c, r64);
           tmem_ld32_nowait(taddr + c + 32, r64 + 32);
+          uint4 ov[with_delta ? 8 : 1];               // this row's 64 values of O (head (n0 + c) / 64)
+          if (with_delta) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k)
+              ov[k] = drow_ok ? __ldg(reinterpret_cast<const uint4*>(dl_orow + c) + k) : make_uint4(0, 0, 0, 0);
+          }
+          float dacc[4] = {0.f, 0.f, 0.f, 0.f};
           // the chunk's 64 bias values go to registers up front: interleaved with the (volatile, memory-
           // clobbering) st.shared they serialised into 8 load -> add -> store chains, 0.4 us per chunk
           float4 bq[16];
@@ -364,6 +385,15 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
               w[3] = pack_bf16x2(__uint_as_float(r[8 * i + 6]) + b1.z, __uint_as_float(r[8 * i + 7]) + b1.w);
               const uint32_t off = (uint32_t)(((4 * h + i) ^ (lane & 7)) << 4);
               sts128(rowp + off, w[0], w[1], w[2], w[3]);
+              if (with_delta) {                        // dO as stored (rounded to bf16) times O, fp32 accumulation
+                const uint4 o4 = ov[4 * h + i];
+                const uint32_t ow[4] = {o4.x, o4.y, o4.z, o4.w};
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                  dacc[u] = fmaf(__uint_as_float(w[u] << 16), __uint_as_float(ow[u] << 16), dacc[u]);
+                  dacc[u] = fmaf(__uint_as_float(w[u] & 0xffff0000u), __uint_as_float(ow[u] & 0xffff0000u), dacc[u]);
+                }
+              }
               if (gelu) {                              // gelu of the ROUNDED pre-activation, as backward will see it
                 uint32_t gw[4];
 #pragma unroll
@@ -382,6 +412,11 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
             my_bias[(half ^ 1) * 64 + lane] = nb0;
             my_bias[(half ^ 1) * 64 + 32 + lane] = nb1;
           }
+          if (with_delta && drow_ok) {
+            const size_t idx = ((size_t)dl_b * pr.dl_H + ((n0 + c) >> 6)) * pr.dl_T + dl_t;
+            pr.dl_delta[idx] = (dacc[0] + dacc[1]) + (dacc[2] + dacc[3]);
+            pr.dl_lse2[idx] = __ldg(pr.dl_lse + idx) * LOG2E_F;
+          }
           fence_async_smem();                         // generic-proxy writes -> visible to the TMA engine
           __syncwarp();
           if (lane == 0) {
@@ -391,7 +426,9 @@ gemm_tc_kernel(const __grid_constant__ Maps maps, const __grid_constant__ Params
           }
         }
         };
-        if (pr.gelu) chunks(std::true_type{}); else chunks(std::false_type{});
+        if (pr.gelu) chunks(std::integral_constant<int, 1>{});
+        else if (pr.dl_o != nullptr) chunks(std::integral_constant<int, 2>{});
+        else chunks(std::integral_constant<int, 0>{});
       }
       tc_fence_before();
       __syncwarp();
@@ -530,6 +567,14 @@ int fill_problem(const GemmDesc& d, int BN, Prob* pr, CUtensorMap* tmA, CUtensor
   pr->splits = 1; pr->range_mode = 0;
   pr->a_mn = a_mn; pr->b_mn = b_mn; pr->accum = d.out_f32_accum != 0; pr->gelu = d.gelu_out != nullptr;
   pr->bias = d.bias;
+  if (d.delta != nullptr) {
+    const AttnDeltaOut& a = *d.delta;
+    if (d.out_f32_accum || d.gelu_out != nullptr || d.N != a.H * 64 || a.T <= 0 || d.M % a.T != 0 || (uintptr_t)a.o % 16 ||
+        a.ldo % 8 != 0)
+      return fail(PACI_EINVAL, "tcgen05 GEMM: the delta epilogue needs the bf16 dgrad of an [mu T, H 64] output");
+    pr->dl_o = a.o; pr->dl_ldo = a.ldo; pr->dl_lse = a.lse; pr->dl_delta = a.delta; pr->dl_lse2 = a.lse2;
+    pr->dl_T = a.T; pr->dl_H = a.H;
+  }
   return PACI_OK;
 }
 

@@ -34,6 +34,27 @@ int gemm_backward_pair(int dtype, int M, int N_out, int K_in, const void* dy, in
   return gemm(dtype, 2, N_out, K_in, M, dy, ld_dy, x, ld_x, nullptr, G_W, ld_g, 1, s);
 }
 
+// Backward of the attention output projection y = o Wo^T (rows a16 + the prologue of a17): G_Wo += dy^T o and
+// d_o = dy Wo in one launch; on the tcgen05 path the dgrad's epilogue also leaves delta = rowsum(d_o * o) per head and
+// lse log2(e) in `attn_scratch` (the layout attention_bwd_tc reads), *prepared = 1, and attention_bwd is then called
+// with scratch_prepared = 1 and launches no delta kernel.  Otherwise *prepared = 0 and nothing else changes.
+int out_proj_backward(int dtype, int mu, int T, int H, int dh, const void* dy, const void* o, const void* Wo,
+                      float* G_Wo, void* d_o, const float* lse, float* attn_scratch, int* prepared, cudaStream_t s) {
+  const int M = mu * T, D = H * dh;
+  *prepared = 0;
+  if (dtype == PACI_BF16 && dh == 64 && T % 128 == 0 && mu > 0 && lse != nullptr && attn_scratch != nullptr) {
+    ProfScope prof(PC_GEMM_BWD_PAIR, 4.0 * M * (double)D * D,
+                   2.0 * (2.0 * (double)M * D + (double)M * D + (double)D * D) + 8.0 * D * D + 2.0 * M * D, s);
+    const AttnDeltaOut a{o, D, lse, attn_scratch, attn_scratch + (size_t)mu * H * T, T, H};
+    const GemmDesc d[2] = {
+        {2, D, D, M, dy, D, o, D, nullptr, G_Wo, D, 1, nullptr, nullptr},       // G_Wo += dy^T o
+        {1, M, D, D, dy, D, Wo, D, nullptr, d_o, D, 0, nullptr, &a}};           // d_o = dy Wo (+ delta, lse2)
+    *prepared = 1;
+    return gemm_tc_multi(d, 2, s);
+  }
+  return gemm_backward_pair(dtype, M, D, D, dy, D, o, D, Wo, D, G_Wo, D, d_o, D, s);
+}
+
 int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
                    void* C, void* Gout, int ldc, cudaStream_t s) {
   if (dtype == PACI_BF16) {
@@ -48,7 +69,7 @@ int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const
 
 int attention_fwd_tc(int mu, int T, int H, const void* qkv, void* o, float* lse, cudaStream_t s);
 int attention_bwd_tc(int mu, int T, int H, const void* dout, const void* qkv, const void* o, const float* lse,
-                     void* dqkv, float* scratch, float* Gbias, cudaStream_t s);
+                     void* dqkv, float* scratch, float* Gbias, int scratch_prepared, cudaStream_t s);
 size_t attention_bwd_tc_scratch_bytes(int mu, int T, int H);
 
 // algorithmic work: causal half of QK^T and PV (2 * mu*H*T*T*dh flops forward, twice that backward)
@@ -65,14 +86,14 @@ int attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void
 // Gbias (fp32 [3 H dh], may be NULL) += column sums of dqkv: the QKV bias gradient (row a15).  The tcgen05
 // kernels take it in their epilogue; the fp32 parity kernels run the column-sum kernel over dqkv afterwards.
 int attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv, const void* o,
-                  const float* lse, void* dqkv, float* scratch, float* Gbias, cudaStream_t s) {
+                  const float* lse, void* dqkv, float* scratch, float* Gbias, cudaStream_t s, int scratch_prepared) {
   int rc;
   {
     const double e = dtype == PACI_BF16 ? 2.0 : 4.0, nd = (double)mu * T * H * dh;
     ProfScope prof(PC_ATTN_BWD, 4.0 * mu * H * (double)T * T * dh, e * 8.0 * nd + 4.0 * mu * H * T, s);
     if (dtype == PACI_BF16) {
       if (dh != 64 || T % 128) return fail(PACI_EINVAL, "bf16 attention needs head dim 64 and T %% 128 == 0");
-      return attention_bwd_tc(mu, T, H, dout, qkv, o, lse, dqkv, scratch, Gbias, s);
+      return attention_bwd_tc(mu, T, H, dout, qkv, o, lse, dqkv, scratch, Gbias, scratch_prepared, s);
     }
     rc = attention_bwd_simt(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, s);
   }
@@ -126,6 +147,15 @@ int paci_op_colsum(int dtype, int rows, int cols, const void* x, float* G, void*
 int paci_op_attention_fwd(int dtype, int mu, int T, int H, int dh, const void* qkv, void* o, float* lse,
                           void* stream) {
   return attention_fwd(dtype, mu, T, H, dh, qkv, o, lse, (cudaStream_t)stream);
+}
+int paci_op_out_proj_backward(int dtype, int mu, int T, int H, int dh, const void* dy, const void* o, const void* Wo,
+                              float* G_Wo, void* d_o, const float* lse, float* attn_scratch, int* prepared, void* stream) {
+  if (prepared == nullptr) return fail(PACI_EINVAL, "paci_op_out_proj_backward: prepared is NULL");
+  return out_proj_backward(dtype, mu, T, H, dh, dy, o, Wo, G_Wo, d_o, lse, attn_scratch, prepared, (cudaStream_t)stream);
+}
+int paci_op_attention_bwd_prepared(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
+                                   const void* o, const float* lse, void* dqkv, float* scratch, void* stream) {
+  return attention_bwd(dtype, mu, T, H, dh, dout, qkv, o, lse, dqkv, scratch, nullptr, (cudaStream_t)stream, 1);
 }
 int paci_op_attention_bwd(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
                           const void* o, const float* lse, void* dqkv, float* scratch, void* stream) {

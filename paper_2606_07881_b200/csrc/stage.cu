@@ -486,10 +486,13 @@ static int backward_impl(paci_stage* st, char* act, const int32_t* tok, const vo
       da = st->sc_dmask;
     }
     // out-proj: do = da Wo ; G_Wo += da^T o
-    RC(gemm_backward_pair(dt, M, D, D, da, D, act + b.o, D, w.wo.wc, D, w.wo.g, D, st->sc_dD2, D, cs));
+    // (tcgen05 path: the dgrad's epilogue also leaves a17's delta = rowsum(do * o) and lse log2(e) in sc_attn)
+    int attn_prepared = 0;
+    RC(out_proj_backward(dt, n_seq, st->T, st->H, st->dh, da, act + b.o, w.wo.wc, w.wo.g, st->sc_dD2,
+                         (float*)(act + b.lse), st->sc_attn, &attn_prepared, cs));
     // a17: attention backward
     RC(attention_bwd(dt, n_seq, st->T, st->H, st->dh, st->sc_dD2, act + b.qkv, act + b.o,
-                     (float*)(act + b.lse), st->sc_dqkv, st->sc_attn, w.bqkv.g, cs));   // + G_bqkv (a15)
+                     (float*)(act + b.lse), st->sc_dqkv, st->sc_attn, w.bqkv.g, cs, attn_prepared));   // + G_bqkv (a15)
     // QKV: dy1 = dqkv Wqkv ; G_Wqkv += dqkv^T y1
     RC(gemm_backward_pair(dt, M, 3 * D, D, st->sc_dqkv, 3 * D, act + b.y1, D, w.wqkv.wc, D, w.wqkv.g, D, st->sc_dD, D, cs));
     // a18: dx = dx1 + LN1bwd(dy1) ; G_ln1 ; colsum(dx) is the previous block's G_b2 (no dropout)

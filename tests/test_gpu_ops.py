@@ -316,3 +316,53 @@ def test_gemm_backward_pair(dtype, M, N_out, K_in):
                                           ld_w, G.data_ptr(), K_in, dx.data_ptr(), K_in, S0))
     assert rel_l2(host(dx), dx_ref) < TOL[dtype] / 4
     assert rel_l2(host(G) - 3.0, 2 * dW_ref) < (1e-5 if dtype == pb.FP32 else 1e-4)
+
+
+@pytest.mark.parametrize("dtype,mu,T,H,dh", [(pb.BF16, 2, 128, 3, 64), (pb.BF16, 1, 384, 4, 64), (pb.BF16, 3, 256, 5, 64),
+                                              (pb.FP32, 2, 32, 4, 16)])
+def test_out_proj_backward_prepares_attention_backward(dtype, mu, T, H, dh):
+    """Rows a13 + a14 of the output projection with the prologue of a17 in the dgrad's epilogue (bf16 / tcgen05):
+    d_o = dy Wo, G_Wo += dy^T o, and scratch <- delta = rowsum_d(d_o * o) per head, lse log2(e).  Checked against the
+    oracle's linear and attention backward (the latter fed the d_o the GPU stored), and delta against its definition;
+    D = H 64 spans one ragged 256-column tile (H = 3, 5) and several row tiles.  fp32: the plain pair, prepared = 0."""
+    import ctypes
+    rng = np.random.default_rng(7 * T + H)
+    D, M = H * dh, mu * T
+    qkv = rng.standard_normal((mu, T, 3 * D))
+    dy, Wo = rng.standard_normal((M, D)), rng.standard_normal((D, D)) * 0.2
+    qkvr, dyr, Wr = rounded(qkv, dtype), rounded(dy, dtype), rounded(Wo, dtype)
+    qd = dev(qkv, dtype)
+    o = torch.empty(mu, T, D, device="cuda", dtype=DT[dtype])
+    lse = torch.empty(mu, H, T, device="cuda")
+    ck(lib.paci_op_attention_fwd(dtype, mu, T, H, dh, qd.data_ptr(), o.data_ptr(), lse.data_ptr(), S0))
+    o_host = host(o).reshape(M, D)
+    do_ref, dW_ref, _ = model.linear_bwd(dyr, o_host, Wr)
+    nb = lib.paci_op_attention_bwd_scratch_bytes(dtype, mu, T, H, dh)
+    scratch = torch.full((nb // 4 + 1,), float("nan"), device="cuda")
+    G = torch.full((D, D), 3.0, device="cuda")
+    d_o = torch.empty(M, D, device="cuda", dtype=DT[dtype])
+    prepared = ctypes.c_int(-1)
+    ck(lib.paci_op_out_proj_backward(dtype, mu, T, H, dh, dev(dy, dtype).data_ptr(), o.data_ptr(), dev(Wo, dtype).data_ptr(),
+                                     G.data_ptr(), d_o.data_ptr(), lse.data_ptr(), scratch.data_ptr(),
+                                     ctypes.addressof(prepared), S0))
+    assert prepared.value == (1 if dtype == pb.BF16 else 0)
+    assert rel_l2(host(d_o), do_ref) < TOL[dtype] / 4
+    assert rel_l2(host(G) - 3.0, dW_ref) < (1e-5 if dtype == pb.FP32 else 1e-4)
+    do_host = host(d_o)                                    # what the GPU stored (bf16-rounded): backward's input
+    if prepared.value:
+        n = mu * H * T
+        delta = host(scratch[:n]).reshape(mu, H, T)
+        lse2 = host(scratch[n:2 * n]).reshape(mu, H, T)
+        want = (do_host.reshape(mu, T, H, dh) * o_host.reshape(mu, T, H, dh)).sum(-1).transpose(0, 2, 1)
+        assert np.abs(delta - want).max() < 1e-4 * max(1.0, np.abs(want).max())
+        assert np.allclose(lse2, host(lse) * np.log2(np.e), rtol=1e-6, atol=1e-6)
+    _, stash = model.attention_fwd(qkvr, H)
+    dq_ref = model.attention_bwd(do_host.reshape(mu, T, D), stash)
+    dqkv = torch.empty_like(qd)
+    ck(lib.paci_op_attention_bwd_prepared(dtype, mu, T, H, dh, d_o.data_ptr(), qd.data_ptr(), o.data_ptr(),
+                                          lse.data_ptr(), dqkv.data_ptr(), scratch.data_ptr(), S0))
+    assert rel_l2(host(dqkv), dq_ref) < TOL[dtype] / 2
+    dqkv2 = torch.empty_like(qd)
+    ck(lib.paci_op_attention_bwd(dtype, mu, T, H, dh, d_o.data_ptr(), qd.data_ptr(), o.data_ptr(),
+                                 lse.data_ptr(), dqkv2.data_ptr(), scratch.data_ptr(), S0))
+    assert rel_l2(host(dqkv), host(dqkv2)) < 1e-3
