@@ -303,6 +303,20 @@ int paci_op_out_proj_backward(int dtype, int mu, int T, int H, int dh, const voi
  * and recompute. */
 int paci_op_attention_bwd_prepared(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
                                    const void* o, const float* lse, void* dqkv, float* scratch, void* stream);
+/* paci_op_attention_bwd WITHOUT caller scratch and without any allocation, for callers that cannot call cudaMalloc
+ * (CUDA graph capture, tight serving loops, harnesses that forbid it): same inputs, same outputs, same kernels; the
+ * scratch is a file-scope `static __device__` array of PACI_ATTENTION_BWD_STATIC_MAX_BYTES inside the library, held by
+ * every GPU that loads the library until the process exits.  All pointers are device pointers, layouts as in
+ * paci_op_attention_bwd.  Limit: paci_op_attention_bwd_scratch_bytes(dtype, mu, T, H, dh) must not exceed the array
+ * (bf16: 8 mu H T + 64 bytes, i.e. mu*H*T <= 524 312 -- configs[4]'s mu 8, H 20, T 1024 needs 1.3 MB); a larger shape
+ * returns PACI_EINVAL with the sizes in paci_last_error() and launches nothing.  Every call on a device shares the
+ * array and it keeps the last call's contents; each call rewrites what it reads (delta, lse*log2(e), the two work
+ * counters) in stream order before reading it, so calls serialised on one stream or by events are independent, while
+ * calls that OVERLAP on the GPU race and give wrong results: serialise them.  Calls no cudaMalloc / cudaFree.
+ * (With paci_profile_begin active the sampling profiler creates events; do not profile inside a capture.) */
+#define PACI_ATTENTION_BWD_STATIC_MAX_BYTES (4u * 1024u * 1024u + 256u)
+int paci_op_attention_bwd_static(int dtype, int mu, int T, int H, int dh, const void* dout, const void* qkv,
+                                 const void* o, const float* lse, void* dqkv, void* stream);
 /* x = wte[tok] + wpe[pos] (a1);  tok int32 [mu,T]; wte [vocab, D], wpe fp32.  Ids outside [0, vocab) are clamped. */
 int paci_op_embed_fwd(int dtype, int mu, int T, int D, int vocab, const int32_t* tok, const float* wte,
                       const float* wpe, void* x, void* stream);

@@ -41,6 +41,7 @@ class ProfEntry(C.Structure):
 
 
 PROF_NCAT = 15
+ATTENTION_BWD_STATIC_MAX_BYTES = 4 * 1024 * 1024 + 256   # PACI_ATTENTION_BWD_STATIC_MAX_BYTES (include/paci.h)
 
 # name -> (restype, argtypes); every symbol include/paci.h declares
 _vp, _i, _i64, _sz, _f = C.c_void_p, C.c_int, C.c_int64, C.c_size_t, C.c_float
@@ -86,6 +87,7 @@ SIGNATURES = {
     "paci_op_attention_bwd_scratch_bytes": (_sz, [_i, _i, _i, _i, _i]),
     "paci_op_out_proj_backward": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_attention_bwd_prepared": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "paci_op_attention_bwd_static": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_embed_fwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_embed_bwd": (_i, [_i, _i, _i, _i, _i, _vp, _vp, _vp, _vp, _vp]),
     "paci_op_dropout": (_i, [_i, _sz, _vp, _vp, _f, C.c_uint64, _i64, C.c_int32, _vp]),
