@@ -562,6 +562,160 @@ def run_k_sweep(args, c, name):
     return 0
 
 
+# ------------------------------------------------------------------------------------ energy per op
+class PowerSampler:
+    """mean board power / SM clock while one op runs back to back (nvidia-smi -lms 50)."""
+
+    def __init__(self, gpu_index):
+        self.gpu = gpu_index
+
+    def __enter__(self):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={self.gpu}", "--query-gpu=power.draw,clocks.sm",
+                                       "--format=csv,noheader,nounits", "-lms", "50"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+        return self
+
+    def __exit__(self, *exc):
+        w, mhz = [], []
+        if self.p is not None:
+            self.p.terminate()
+            try:
+                self.p.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.p.kill()
+            self.f.flush()
+            self.f.seek(0)
+            for line in self.f.read().splitlines():
+                parts = [x.strip() for x in line.split(",")]
+                try:
+                    w.append(float(parts[0])); mhz.append(float(parts[1]))
+                except (ValueError, IndexError):
+                    continue
+        self.f.close()
+        os.unlink(self.f.name)
+        n = len(w) // 3                                    # drop the ramp: keep the last two thirds
+        w, mhz = w[n:], mhz[n:]
+        self.watts = sum(w) / len(w) if w else None
+        self.mhz = sum(mhz) / len(mhz) if mhz else None
+        return False
+
+
+def run_energy(args, c, name):
+    """`--energy`: every kernel of one block at the config's shapes, run alone and back to back for ~2.5 s each under
+    the board's power cap: mean W, SM clock, us per call and mJ per call (= W x us), with cuBLAS (torch) on the same
+    GEMM shapes beside ours.  The step is power-capped, so mJ per call is what a kernel costs it."""
+    import ctypes
+    import torch
+    from paper_2606_07881_b200 import binding as pb
+    lib = pb.lib
+    torch.cuda.set_device(0)
+    bf = torch.bfloat16
+    D, H, T, mu = c["D"], c["H"], c["T"], c["mu"]
+    M = mu * T
+    S0 = lambda: torch.cuda.current_stream().cuda_stream
+    rows = []
+
+    def run(label, fn, flops=None, secs=2.5):
+        for _ in range(20):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n, t0 = 0, time.time()
+        with PowerSampler(0) as ps:
+            e0.record()
+            while time.time() - t0 < secs:
+                for _ in range(200):
+                    fn()
+                n += 200
+                torch.cuda.synchronize()
+            e1.record()
+            torch.cuda.synchronize()
+        us = e0.elapsed_time(e1) * 1e3 / n
+        r = {"op": label, "watts": ps.watts, "sm_mhz": ps.mhz, "us_per_call": round(us, 2),
+             "mj_per_call": round(ps.watts * us * 1e-3, 2) if ps.watts else None}
+        if flops:
+            r["tflops"] = round(flops / us * 1e-6, 1)
+        rows.append(r)
+        time.sleep(0.5)
+
+    def rnd(*shape, scale=1.0):
+        return (torch.randn(*shape, device="cuda") * scale).to(bf)
+
+    keep = []                                              # tensors whose data_ptr() the closures captured
+
+    def ours_fwd(N, K, gelu=False):
+        A, B, bias = rnd(M, K), rnd(N, K, scale=0.02), torch.randn(N, device="cuda")
+        Cc, G = torch.empty(M, N, device="cuda", dtype=bf), torch.empty(M, N, device="cuda", dtype=bf)
+        keep.extend([A, B, bias, Cc, G])
+        if gelu:
+            return lambda: lib.paci_op_gemm_bias_gelu(pb.BF16, M, N, K, A.data_ptr(), K, B.data_ptr(), K, bias.data_ptr(),
+                                                      Cc.data_ptr(), G.data_ptr(), N, S0())
+        return lambda: lib.paci_op_gemm(pb.BF16, 0, M, N, K, A.data_ptr(), K, B.data_ptr(), K, bias.data_ptr(),
+                                        Cc.data_ptr(), N, 0, S0())
+
+    def cublas_fwd(N, K):
+        A, B, bias = rnd(M, K), rnd(N, K, scale=0.02), rnd(N)
+        keep.extend([A, B, bias])
+        return lambda: torch.nn.functional.linear(A, B, bias)
+
+    def ours_pair(N_out, K_in):
+        dy, x, W = rnd(M, N_out), rnd(M, K_in), rnd(N_out, K_in, scale=0.02)
+        G, dx = torch.zeros(N_out, K_in, device="cuda"), torch.empty(M, K_in, device="cuda", dtype=bf)
+        keep.extend([dy, x, W, G, dx])
+        return lambda: lib.paci_op_gemm_backward_pair(pb.BF16, M, N_out, K_in, dy.data_ptr(), N_out, x.data_ptr(), K_in,
+                                                      W.data_ptr(), K_in, G.data_ptr(), K_in, dx.data_ptr(), K_in, S0())
+
+    def cublas_pair(N_out, K_in):                          # the same two products, both with bf16 outputs
+        dy, x, W = rnd(M, N_out), rnd(M, K_in), rnd(N_out, K_in, scale=0.02)
+        keep.extend([dy, x, W])
+
+        def f():
+            torch.matmul(dy, W)
+            torch.matmul(dy.t(), x)
+        return f
+
+    for label, N, K, gelu in (("QKV forward", 3 * D, D, False), ("out-proj forward", D, D, False),
+                              ("MLP-up forward + GELU epilogue", 4 * D, D, True), ("MLP-down forward", D, 4 * D, False)):
+        run(f"gemm_tc {label} {M}x{N}x{K}", ours_fwd(N, K, gelu), 2.0 * M * N * K)
+        run(f"cuBLAS  F.linear {M}x{N}x{K}" + (" (no GELU)" if gelu else ""), cublas_fwd(N, K), 2.0 * M * N * K)
+    for label, N_out, K_in in (("Wqkv", 3 * D, D), ("W1", 4 * D, D), ("W2", D, 4 * D), ("Wo", D, D)):
+        run(f"gemm_tc backward pair {label} (dgrad + fp32 wgrad accumulate)", ours_pair(N_out, K_in), 4.0 * M * N_out * K_in)
+        run(f"cuBLAS  dgrad + wgrad {label} (two matmuls, bf16 out)", cublas_pair(N_out, K_in), 4.0 * M * N_out * K_in)
+    qkv, do = rnd(mu, T, 3 * D), rnd(mu, T, D)
+    o, lse, dqkv = torch.empty(mu, T, D, device="cuda", dtype=bf), torch.empty(mu, H, T, device="cuda"), torch.empty_like(qkv)
+    scratch = torch.empty(lib.paci_op_attention_bwd_scratch_bytes(pb.BF16, mu, T, H, D // H), device="cuda", dtype=torch.uint8)
+    fl = 2.0 * mu * H * T * T * (D // H)
+    run("attention forward", lambda: lib.paci_op_attention_fwd(pb.BF16, mu, T, H, D // H, qkv.data_ptr(), o.data_ptr(),
+                                                               lse.data_ptr(), S0()), fl)
+    run("attention backward", lambda: lib.paci_op_attention_bwd(pb.BF16, mu, T, H, D // H, do.data_ptr(), qkv.data_ptr(),
+                                                                o.data_ptr(), lse.data_ptr(), dqkv.data_ptr(),
+                                                                scratch.data_ptr(), S0()), 2 * fl)
+    x, res, g, b = rnd(M, D), rnd(M, D), torch.randn(D, device="cuda"), torch.randn(D, device="cuda")
+    xs, y, dx = torch.empty_like(x), torch.empty_like(x), torch.empty_like(x)
+    mean, rstd = torch.empty(M, device="cuda"), torch.empty(M, device="cuda")
+    Gg, Gb, Gc = (torch.zeros(D, device="cuda") for _ in range(3))
+    run("LayerNorm forward (+ residual)", lambda: lib.paci_op_layernorm_fwd(
+        pb.BF16, M, D, x.data_ptr(), res.data_ptr(), g.data_ptr(), b.data_ptr(), xs.data_ptr(), y.data_ptr(),
+        mean.data_ptr(), rstd.data_ptr(), S0()))
+    run("LayerNorm backward (+ residual, column sums)", lambda: lib.paci_op_layernorm_bwd(
+        pb.BF16, M, D, y.data_ptr(), xs.data_ptr(), mean.data_ptr(), rstd.data_ptr(), g.data_ptr(), res.data_ptr(),
+        dx.data_ptr(), Gg.data_ptr(), Gb.data_ptr(), Gc.data_ptr(), S0()))
+    dg, pp = rnd(M, 4 * D), rnd(M, 4 * D)
+    dp, Gb4 = torch.empty_like(pp), torch.zeros(4 * D, device="cuda")
+    run("GELU backward + b1 column sums", lambda: lib.paci_op_gelu_bwd(pb.BF16, M, 4 * D, dg.data_ptr(), pp.data_ptr(),
+                                                                       dp.data_ptr(), Gb4.data_ptr(), S0()))
+    per_block = sum(r["mj_per_call"] or 0.0 for r in rows if not r["op"].startswith("cuBLAS"))
+    per_block += sum((r["mj_per_call"] or 0.0) for r in rows if r["op"].startswith("LayerNorm"))   # two of each per block
+    print(json.dumps({"metric": "energy per kernel call under the board's power cap", "n_gpus": 1,
+                      "config": {"workload": workload_name(name, c)}, "data": "synthetic (N(0,1) activations)",
+                      "dtype": "bf16", "mj_per_block_fwd_bwd": round(per_block, 1), "ops": rows}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -578,10 +732,14 @@ def main():
                     help="auto: also run App. D.5's partitioner on this build's own per-layer profile and report "
                          "the partitioned pipeline as an EXTRA (the headline stays on BASELINE.json's equal split)")
     ap.add_argument("--k-sweep", action="store_true", help="BASELINE.json configs[3]: k in {1,2,4,8}, PACI vs flush")
+    ap.add_argument("--energy", action="store_true",
+                    help="W, SM clock, us and mJ per call of every block kernel run alone under the power cap, cuBLAS beside")
     args = ap.parse_args()
     c = CONFIGS[args.config]
     if args.impl == "reference":
         return run_reference(args, c, args.config)
+    if args.energy:
+        return run_energy(args, c, args.config)
     if args.k_sweep:
         return run_k_sweep(args, CONFIGS["medium8"] if args.config == "medium" else c, "medium8" if args.config == "medium" else args.config)
     return run_ours(args, c, args.config)
