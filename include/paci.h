@@ -205,7 +205,8 @@ int paci_pipeline_destroy(paci_pipeline_t* p);
 /* Run n_microbatches through the pipeline in the canonical logical schedule: per logical
  * slot every stage does at most one op, a message produced in slot tau is visible in slot tau+1,
  * backward before forward; the admission rule is enforced by paci_forward itself.
- *   tokens: int32 [n_microbatches, mu, T+1]; column t+1 is the target of column t.
+ *   tokens: int32 [n_microbatches, mu, T+1]; column t+1 is the target of column t.  n_microbatches = 0 is a no-op
+ *           (tokens may be NULL): nothing is launched, no update happens, the report has 0 slots and launches.
  *           tokens_on_host = 0: DEVICE pointer.  1: HOST pointer (pinned or pageable); the run then
  *           includes the host->device copy of every micro-batch's tokens and the device->host read
  *           of its loss.

@@ -11,6 +11,11 @@ namespace paci {
 
 int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, const void* B, int ldb,
          const float* bias, void* C, int ldc, int out_f32_accum, cudaStream_t s) {
+  if (M <= 0 || N <= 0) return PACI_OK;                 // empty output
+  if (K <= 0) {                                         // empty contraction: nothing to add; an overwrite has no value
+    if (out_f32_accum) return PACI_OK;
+    return fail(PACI_EINVAL, "gemm: K = %d with an overwritten output", K);
+  }
   const double e = dtype == PACI_BF16 ? 2.0 : 4.0;
   ProfScope prof(layout == 0 ? PC_GEMM_FWD : layout == 1 ? PC_GEMM_DGRAD : PC_GEMM_WGRAD, 2.0 * M * N * K,
                  e * ((double)M * K + (double)N * K) + (out_f32_accum ? 8.0 : e) * M * N, s);
@@ -21,6 +26,7 @@ int gemm(int dtype, int layout, int M, int N, int K, const void* A, int lda, con
 
 int gemm_backward_pair(int dtype, int M, int N_out, int K_in, const void* dy, int ld_dy, const void* x, int ld_x,
                        const void* W, int ld_w, float* G_W, int ld_g, void* dx, int ld_dx, cudaStream_t s) {
+  if (M <= 0 || N_out <= 0 || K_in <= 0) return PACI_OK;   // no tokens: dx is empty and G_W gets nothing
   if (dtype == PACI_BF16) {
     ProfScope prof(PC_GEMM_BWD_PAIR, 4.0 * M * (double)N_out * K_in,
                    2.0 * (2.0 * (double)M * N_out + (double)M * K_in + (double)N_out * K_in) + 8.0 * N_out * K_in + 2.0 * M * K_in, s);
@@ -57,6 +63,8 @@ int out_proj_backward(int dtype, int mu, int T, int H, int dh, const void* dy, c
 
 int gemm_bias_gelu(int dtype, int M, int N, int K, const void* A, int lda, const void* B, int ldb, const float* bias,
                    void* C, void* Gout, int ldc, cudaStream_t s) {
+  if (M <= 0 || N <= 0) return PACI_OK;
+  if (K <= 0) return fail(PACI_EINVAL, "gemm_bias_gelu: K = %d", K);
   if (dtype == PACI_BF16) {
     ProfScope prof(PC_GEMM_FWD, 2.0 * M * N * K, 2.0 * ((double)M * K + (double)N * K) + 4.0 * M * N, s);
     return gemm_tc(0, M, N, K, A, lda, B, ldb, bias, C, ldc, 0, s, Gout);

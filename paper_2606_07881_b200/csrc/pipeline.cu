@@ -145,7 +145,7 @@ int paci_pipeline_run(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_
 int paci_pipeline_run_var(paci_pipeline_t* p, const int32_t* tokens, int32_t tokens_on_host, int64_t n,
                           const int32_t* n_seq, int32_t mode, float lr, const float* lr_by_update,
                           int64_t n_updates, void* stream, paci_run_report* rep) {
-  if (!p || !tokens || !rep) return fail(PACI_EINVAL, "null pointer");
+  if (!p || !rep || (!tokens && n > 0)) return fail(PACI_EINVAL, "null pointer");   // n = 0: tokens may be NULL
   if (n < 0 || n > MAX_MB) return fail(PACI_EINVAL, "n_microbatches %lld out of range", (long long)n);
   if (mode != PACI_MODE_PACI && mode != PACI_MODE_FLUSH) return fail(PACI_EINVAL, "mode %d", mode);
   if (n_seq)

@@ -90,3 +90,18 @@ def test_checkpoint_and_dropout_config_validation(pb):
                 pb.make_config(0, 2, 1, 64, 4, 32, 2, 4, 256, pb.FP32, dropout_p=1.0),
                 pb.make_config(0, 2, 1, 128, 2, 64, 2, 4, 256, pb.BF16)):     # bf16: T % 128
         assert pb.lib.paci_stage_workspace_bytes(C.byref(bad)) == 0
+
+
+def test_empty_shapes_are_decided_on_the_host():
+    """Empty outputs and empty contractions never reach a kernel (so this runs without a GPU): an empty output or an
+    accumulate over zero tokens is PACI_OK, an OVERWRITE from an empty contraction has no value and is PACI_EINVAL."""
+    from paper_2606_07881_b200 import binding as pb
+    lib = pb.lib
+    p = 256                                                  # never dereferenced
+    for dt in (pb.FP32, pb.BF16):
+        assert lib.paci_op_gemm(dt, 0, 0, 64, 64, p, 64, p, 64, None, p, 64, 0, None) == 0
+        assert lib.paci_op_gemm(dt, 2, 64, 64, 0, p, 64, p, 64, None, p, 64, 1, None) == 0
+        assert lib.paci_op_gemm(dt, 0, 8, 64, 0, p, 64, p, 64, None, p, 64, 0, None) == -1
+        assert b"K = 0" in lib.paci_last_error()
+        assert lib.paci_op_gemm_backward_pair(dt, 0, 64, 64, p, 64, p, 64, p, 64, p, 64, p, 64, None) == 0
+        assert lib.paci_op_layernorm_fwd(dt, 0, 64, p, None, p, p, None, p, p, p, None) == 0
