@@ -416,6 +416,9 @@ static int forward_impl(paci_stage* st, char* act, const void* x, const int32_t*
     // a7 + a8: p = y2 W1^T + b1 (stashed: backward needs gelu'(p)) and g = gelu(p), one launch in bf16 mode (the
     // activation is computed in the GEMM epilogue and leaves through a second TMA store)
     RC(gemm_bias_gelu(dt, M, 4 * D, D, act + b.y2, D, w.w1.wc, D, w.b1.w, act + b.p, act + b.g, 4 * D, cs));
+    // a recomputation (checkpointed backward: out == NULL) of a stage without the head stops here on its last block:
+    // nothing that backward reads comes after g (the MLP-down output only feeds the stage's output)
+    if (l == st->L - 1 && out == nullptr && !st->cfg.has_head) return PACI_OK;
     // a9: m = g W2^T + b2 ; the residual add is fused into the next LayerNorm
     RC(gemm(dt, 0, M, D, 4 * D, act + b.g, 4 * D, w.w2.wc, 4 * D, w.b2.w, st->sc_proj, D, 0, cs));
     if (pd > 0.f) RC(dropout(dt, (size_t)M * D, st->sc_proj, st->sc_proj, pd, seed, mb_id, site_mlp(l), cs));
