@@ -145,9 +145,12 @@ __device__ __forceinline__ float tanh_fast(float u) {
   asm("tanh.approx.f32 %0, %1;" : "=f"(r) : "f"(u));
   return r;
 }
+// gelu(p) = 0.5 p (1 + tanh(C (p + A p^3))) as five FMA-class operations and the tanh: u = p (C + C A p^2),
+// h = 0.5 p, result = h + h tanh(u)
 __device__ __forceinline__ float gelu_bf16(float p) {
-  const float u = 0.7978845608028654f * (p + 0.044715f * p * p * p);
-  return 0.5f * p * (1.f + tanh_fast(u));
+  const float u = p * fmaf(0.7978845608028654f * 0.044715f, p * p, 0.7978845608028654f);
+  const float h = 0.5f * p;
+  return fmaf(h, tanh_fast(u), h);
 }
 
 static inline int ceil_div(long long a, long long b) { return (int)((a + b - 1) / b); }

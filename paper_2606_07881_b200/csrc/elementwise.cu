@@ -787,13 +787,17 @@ int ln_bwd(int dtype, int rows, int D, const void* dy, const void* x, const floa
 template <typename T> __device__ __forceinline__ float tanh_t(float u) { return tanhf(u); }
 template <> __device__ __forceinline__ float tanh_t<bf16>(float u) { return tanh_fast(u); }
 template <typename T> __device__ __forceinline__ float gelu_f(float p) {
-  const float u = GELU_C * (p + GELU_A * p * p * p);
-  return 0.5f * p * (1.f + tanh_t<T>(u));
+  const float u = p * fmaf(GELU_C * GELU_A, p * p, GELU_C);
+  const float h = 0.5f * p;
+  return fmaf(h, tanh_t<T>(u), h);
 }
+// gelu'(p) = 0.5 (1 + th) + (1 - th^2) p (0.5 C + 1.5 C A p^2), th = tanh(p (C + C A p^2)): the same expression as
+// 0.5 (1 + th) + 0.5 p (1 - th^2) C (1 + 3 A p^2), arranged as eight FMA-class operations and the tanh
 template <typename T> __device__ __forceinline__ float dgelu_f(float p) {
-  const float u = GELU_C * (p + GELU_A * p * p * p);
-  const float th = tanh_t<T>(u);
-  return 0.5f * (1.f + th) + 0.5f * p * (1.f - th * th) * GELU_C * (1.f + 3.f * GELU_A * p * p);
+  const float q = p * p;
+  const float th = tanh_t<T>(p * fmaf(GELU_C * GELU_A, q, GELU_C));
+  const float pw = p * fmaf(1.5f * GELU_C * GELU_A, q, 0.5f * GELU_C);
+  return fmaf(fmaf(-th, th, 1.f), pw, fmaf(0.5f, th, 0.5f));
 }
 
 template <typename T>
