@@ -800,6 +800,42 @@ template <typename T> __device__ __forceinline__ float dgelu_f(float p) {
   return fmaf(fmaf(-th, th, 1.f), pw, fmaf(0.5f, th, 0.5f));
 }
 
+// Two elements at a time on sm_100's packed fp32 pairs (FMUL2 / FFMA2: one issue slot for both): the GELU backward
+// kernel is partly ALU-bound, and the derivative is most of its arithmetic.  Same expression as dgelu_f<bf16>.
+__device__ __forceinline__ unsigned long long f2_pack(float lo, float hi) {
+  unsigned long long r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void f2_unpack(unsigned long long v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ unsigned long long f2_mul(unsigned long long a, unsigned long long b) {
+  unsigned long long r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ unsigned long long f2_fma(unsigned long long a, unsigned long long b, unsigned long long c) {
+  unsigned long long r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+// (v0, v1) *= gelu'(p0), gelu'(p1)
+__device__ __forceinline__ void mul_dgelu2_bf16(float& v0, float& v1, float p0, float p1) {
+  const unsigned long long p = f2_pack(p0, p1);
+  const unsigned long long q = f2_mul(p, p);
+  const unsigned long long u = f2_mul(p, f2_fma(f2_pack(GELU_C * GELU_A, GELU_C * GELU_A), q, f2_pack(GELU_C, GELU_C)));
+  float u0, u1;
+  f2_unpack(u, u0, u1);
+  const unsigned long long th = f2_pack(tanh_fast(u0), tanh_fast(u1));
+  const unsigned long long pw = f2_mul(p, f2_fma(f2_pack(1.5f * GELU_C * GELU_A, 1.5f * GELU_C * GELU_A), q,
+                                                 f2_pack(0.5f * GELU_C, 0.5f * GELU_C)));
+  const unsigned long long one = f2_pack(1.f, 1.f), half = f2_pack(0.5f, 0.5f);
+  const unsigned long long nth = f2_mul(th, f2_pack(-1.f, -1.f));
+  const unsigned long long d = f2_fma(f2_fma(nth, th, one), pw, f2_fma(half, th, half));
+  f2_unpack(f2_mul(f2_pack(v0, v1), d), v0, v1);
+}
+
 template <typename T>
 __global__ void __launch_bounds__(256) gelu_fwd_kernel(size_t nvec, const T* __restrict__ p, T* __restrict__ out) {
   PACI_PDL_SYNC;
@@ -870,8 +906,13 @@ __global__ void __launch_bounds__(CS_TX * CS_TY, 2) colslab_kernel(int rows, int
           if (GELU) {
             float pv[V];
             unpack_raw<T>(rp[u], pv);
+            if constexpr (sizeof(T) == 2) {
 #pragma unroll
-            for (int j = 0; j < V; ++j) v[j] *= dgelu_f<T>(pv[j]);
+              for (int j = 0; j < V; j += 2) mul_dgelu2_bf16(v[j], v[j + 1], pv[j], pv[j + 1]);
+            } else {
+#pragma unroll
+              for (int j = 0; j < V; ++j) v[j] *= dgelu_f<T>(pv[j]);
+            }
             store_vec<T>(out + (size_t)r * cols + c, v);
 #pragma unroll
             for (int j = 0; j < V; ++j) v[j] = to_f(from_f<T>(v[j]));  // sum what was stored
