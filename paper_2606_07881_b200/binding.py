@@ -194,9 +194,9 @@ class Stage:
         self.handle = h
         self.act_dtype = torch.bfloat16 if cfg.dtype == BF16 else torch.float32
 
-    def close(self):
+    def close(self, _destroy=lib.paci_stage_destroy):      # bound at definition: module globals are gone at shutdown
         if getattr(self, "handle", None):
-            lib.paci_stage_destroy(self.handle)
+            _destroy(self.handle)
             self.handle = None
 
     __del__ = close
@@ -299,9 +299,9 @@ class Pipeline:
             check(lib.paci_pipeline_create(arr, S, base, nbytes, C.byref(h)), "paci_pipeline_create")
         self.handle = h
 
-    def close(self):
+    def close(self, _destroy=lib.paci_pipeline_destroy):   # bound at definition: module globals are gone at shutdown
         if getattr(self, "handle", None):
-            lib.paci_pipeline_destroy(self.handle)
+            _destroy(self.handle)
             self.handle = None
 
     __del__ = close
